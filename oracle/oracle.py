@@ -1,0 +1,321 @@
+"""oracle/oracle.py — CPU ORACLE of the tensor-tomography gradient path.  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import this.
+It shares no code with the CUDA library and never imports the package's binding.
+
+What is here (numpy, fp64) and what it follows:
+  real_sh / sh_index   real spherical harmonics, textbook definition                PAPER.md:236-238, reading S14
+  q_hat                small-angle scattering direction, Eq. 1 second line
+  basis_matrix         segment average B_{sc,i}, Eq. 3, Gauss-Legendre quadrature
+  basis_forward/adjoint Eq. 6 reciprocal-space map and its transpose
+  forward / adjoint    A = (basis map) o (John transform), Eq. 6-8, and A^T
+  loss_gradient        r = Ac - I (Eq. 13), L = 1/2 sum w r^2, grad = A^T (w r)     PAPER.md:101, 324, readings S10, S11
+The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
+
+Pins: tests/test_oracle_sh.py, tests/test_oracle_john.py, tests/test_oracle_model.py (all CPU).
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+import subprocess
+
+import numpy as np
+from numpy.polynomial import legendre as _leg
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libora.so")
+_lib = None
+
+STANDARD_VECS = {            # Table I, PAPER.md:27-37 (row 2 garbled: reading S1, j = +y, k = +x)
+    "p": (0.0, 0.0, 1.0), "j": (0.0, 1.0, 0.0), "k": (1.0, 0.0, 0.0),
+    "q0": (1.0, 0.0, 0.0), "q90": (0.0, 1.0, 0.0),
+    "inner_axis": (0.0, 1.0, 0.0), "outer_axis": (1.0, 0.0, 0.0),
+}
+
+
+def build(force: bool = False) -> str:
+    """compile oracle/ora.c -> oracle/libora.so (gcc -O2, OpenMP on the embarrassingly parallel loops)."""
+    src = os.path.join(_HERE, "ora.c")
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-o", _LIB_PATH, src, "-lm"])
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB_PATH)
+        dp, fp, ip = (ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int32))
+        L.ora_geom_create.restype = ctypes.c_void_p
+        L.ora_geom_create.argtypes = [ctypes.c_int] * 6 + [dp, dp, dp, dp, dp, ctypes.c_double, ctypes.c_double]
+        L.ora_geom_destroy.argtypes = [ctypes.c_void_p]
+        L.ora_geom_get.argtypes = [ctypes.c_void_p, ctypes.c_int, dp, dp, dp, ctypes.POINTER(ctypes.c_int), dp]
+        L.ora_john_forward.argtypes = [ctypes.c_void_p, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int]
+        L.ora_john_forward_rays.argtypes = [ctypes.c_void_p, fp, ctypes.c_int, ctypes.c_int, ctypes.c_long, ip, dp, ctypes.c_int]
+        L.ora_john_adjoint_scatter.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp]
+        L.ora_john_adjoint_gather.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp, ctypes.c_int]
+        L.ora_john_adjoint_voxels.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, ctypes.c_long, ip, dp, ctypes.c_int]
+        L.ora_voxel_taps.restype = ctypes.c_long
+        L.ora_voxel_taps.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_long]
+        L.ora_dense_matrix.argtypes = [ctypes.c_void_p, ctypes.c_int, dp]
+        _lib = L
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _fp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def _ip(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+
+
+def default_threads() -> int:
+    return len(os.sched_getaffinity(0))
+
+
+# ------------------------------------------------------------------------------------------------
+# geometry + John transform (C)
+# ------------------------------------------------------------------------------------------------
+class Geometry:
+    """Per-projection geometry (A0).  rotations/tilts in radians; offsets in pixels; vecs overrides Table I."""
+
+    def __init__(self, volume_shape, det_shape, rotations, tilts, j_offsets=None, k_offsets=None, vecs=None,
+                 voxel_size=1.0, pixel_size=1.0):
+        L = _load()
+        self.shape = tuple(int(v) for v in volume_shape)
+        self.det = tuple(int(v) for v in det_shape)
+        self.rot = np.ascontiguousarray(rotations, dtype=np.float64)
+        self.tilt = np.ascontiguousarray(tilts, dtype=np.float64)
+        self.P = int(self.rot.size)
+        self.joff = np.zeros(self.P) if j_offsets is None else np.ascontiguousarray(j_offsets, dtype=np.float64)
+        self.koff = np.zeros(self.P) if k_offsets is None else np.ascontiguousarray(k_offsets, dtype=np.float64)
+        v = dict(STANDARD_VECS)
+        if vecs:
+            v.update(vecs)
+        self.vecs = {k: np.asarray(val, dtype=np.float64) for k, val in v.items()}
+        flat = np.concatenate([self.vecs[n] for n in ("p", "j", "k", "inner_axis", "outer_axis")]).astype(np.float64)
+        self.a, self.b = float(voxel_size), float(pixel_size)
+        self._h = L.ora_geom_create(*self.shape, *self.det, self.P, _dp(self.rot), _dp(self.tilt), _dp(self.joff),
+                                    _dp(self.koff), _dp(flat), self.a, self.b)
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.ora_geom_destroy(self._h)
+            self._h = None
+
+    def get(self, s):
+        d, js, ks = np.zeros(3), np.zeros(3), np.zeros(3)
+        m, w = ctypes.c_int(), ctypes.c_double()
+        _load().ora_geom_get(self._h, int(s), _dp(d), _dp(js), _dp(ks), ctypes.byref(m), ctypes.byref(w))
+        return d, js, ks, m.value, w.value
+
+    def rotation_matrix(self, s):
+        """R_s = R_beta(beta_s) R_alpha(alpha_s), PAPER.md:46 (numpy restatement used by the basis builder)."""
+        return _rodrigues(self.vecs["outer_axis"], self.tilt[s]) @ _rodrigues(self.vecs["inner_axis"], self.rot[s])
+
+
+def _rodrigues(n, theta):
+    n = np.asarray(n, dtype=np.float64)
+    Kx = np.array([[0, -n[2], n[1]], [n[2], 0, -n[0]], [-n[1], n[0], 0]])
+    return np.eye(3) * math.cos(theta) + math.sin(theta) * Kx + (1 - math.cos(theta)) * np.outer(n, n)
+
+
+def _vol32(vol, K):
+    vol = np.ascontiguousarray(vol, dtype=np.float32)
+    assert vol.ndim == 4 and vol.shape[3] >= K
+    return vol, vol.shape[3]
+
+
+def john_forward(g: Geometry, vol, K, s0=0, s1=None, threads=None):
+    """proj[s1-s0][J][Kd][K] float64 = Joseph line integrals of the K-channel volume (A1)."""
+    s1 = g.P if s1 is None else s1
+    vol, ldk = _vol32(vol, K)
+    assert vol.shape[:3] == g.shape
+    out = np.empty((s1 - s0,) + g.det + (K,), dtype=np.float64)
+    _load().ora_john_forward(g._h, _fp(vol), K, ldk, s0, s1, _dp(out), threads or default_threads())
+    return out
+
+
+def john_forward_rays(g: Geometry, vol, K, sjk, threads=None):
+    vol, ldk = _vol32(vol, K)
+    sjk = np.ascontiguousarray(sjk, dtype=np.int32).reshape(-1, 3)
+    out = np.empty((sjk.shape[0], K), dtype=np.float64)
+    _load().ora_john_forward_rays(g._h, _fp(vol), K, ldk, sjk.shape[0], _ip(sjk), _dp(out), threads or default_threads())
+    return out
+
+
+def john_adjoint(g: Geometry, y, form="gather", threads=None):
+    """out[X][Y][Z][K] float64 = exact transpose of john_forward applied to y[P][J][Kd][K] (A2)."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    K = y.shape[-1]
+    assert y.shape == (g.P,) + g.det + (K,)
+    out = np.empty(g.shape + (K,), dtype=np.float64)
+    if form == "scatter":
+        _load().ora_john_adjoint_scatter(g._h, _dp(y), K, _dp(out))
+    else:
+        _load().ora_john_adjoint_gather(g._h, _dp(y), K, _dp(out), threads or default_threads())
+    return out
+
+
+def john_adjoint_voxels(g: Geometry, y, xyz, threads=None):
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    K = y.shape[-1]
+    xyz = np.ascontiguousarray(xyz, dtype=np.int32).reshape(-1, 3)
+    out = np.empty((xyz.shape[0], K), dtype=np.float64)
+    _load().ora_john_adjoint_voxels(g._h, _dp(y), K, xyz.shape[0], _ip(xyz), _dp(out), threads or default_threads())
+    return out
+
+
+def voxel_taps(g: Geometry, x, y, z):
+    """rows (s, j, k, P_{sjk,xyz}) of the non-zero entries of the John matrix in the column of voxel (x,y,z)."""
+    cap = 64 * g.P
+    buf = np.empty((cap, 4), dtype=np.float64)
+    n = _load().ora_voxel_taps(g._h, int(x), int(y), int(z), _dp(buf), cap)
+    assert n <= cap
+    return buf[:n].copy()
+
+
+def dense_john_matrix(g: Geometry, s):
+    """[J*Kd][X*Y*Z] dense P_s from the closed form Lambda*Lambda (tiny problems only)."""
+    nv = g.shape[0] * g.shape[1] * g.shape[2]
+    mat = np.empty((g.det[0] * g.det[1], nv), dtype=np.float64)
+    _load().ora_dense_matrix(g._h, int(s), _dp(mat))
+    return mat
+
+
+# ------------------------------------------------------------------------------------------------
+# real spherical harmonics and the segment-integrated basis matrix (numpy)
+# ------------------------------------------------------------------------------------------------
+def sh_index(ell_max: int):
+    """[(l, m)] for even l <= ell_max, l ascending then m = -l..l (reading S14)."""
+    return [(l, m) for l in range(0, ell_max + 1, 2) for m in range(-l, l + 1)]
+
+
+def real_sh(l: int, m: int, n):
+    """Real spherical harmonic Y_lm at unit vectors n[..., 3], 4pi-normalised (sphere mean of Y^2 = 1, Y_00 = 1),
+    no Condon-Shortley phase:  Y_lm = N_l|m| P_l^|m|(cos th) * {sqrt2 cos(m ph) | 1 | sqrt2 sin(|m| ph)} for
+    m > 0 | m = 0 | m < 0, with P_l^m(x) = (1-x^2)^(m/2) d^m/dx^m P_l(x), N_lm = sqrt((2l+1)(l-m)!/(l+m)!)."""
+    n = np.asarray(n, dtype=np.float64)
+    ct = np.clip(n[..., 2], -1.0, 1.0)
+    ph = np.arctan2(n[..., 1], n[..., 0])
+    am = abs(m)
+    plm = (1.0 - ct * ct) ** (0.5 * am) * _leg.Legendre.basis(l).deriv(am)(ct)
+    norm = math.sqrt((2 * l + 1) * math.factorial(l - am) / math.factorial(l + am))
+    if m > 0:
+        return math.sqrt(2.0) * norm * plm * np.cos(m * ph)
+    if m < 0:
+        return math.sqrt(2.0) * norm * plm * np.sin(am * ph)
+    return norm * plm
+
+
+def q_hat(g: Geometry, phi):
+    """lab-frame scattering direction, small-angle line of Eq. 1: cos(phi) q0 + sin(phi) q90."""
+    phi = np.asarray(phi, dtype=np.float64)
+    return np.cos(phi)[..., None] * g.vecs["q0"] + np.sin(phi)[..., None] * g.vecs["q90"]
+
+
+def basis_matrix(g: Geometry, ell_max: int, seg_start, seg_end, n_quad: int = 32, rule: str = "gauss"):
+    """B[P][K][D] float64: B[s][i][c] = mean over [start_c, end_c] of Y_i(R_s^T q(phi))  (Eq. 3).
+    rule = 'gauss' (Gauss-Legendre, n_quad nodes), 'simpson' (composite, n_quad panels) or 'central'
+    (the central-angle approximation the paper mentions)."""
+    seg_start = np.asarray(seg_start, dtype=np.float64)
+    seg_end = np.asarray(seg_end, dtype=np.float64)
+    D = seg_start.size
+    idx = sh_index(ell_max)
+    B = np.zeros((g.P, len(idx), D), dtype=np.float64)
+    if rule == "gauss":
+        xs, ws = _leg.leggauss(n_quad)
+        ws = ws / 2.0                                   # weights of the mean over [-1,1]
+    elif rule == "simpson":
+        xs = np.linspace(-1.0, 1.0, 2 * n_quad + 1)
+        ws = np.ones_like(xs)
+        ws[1:-1:2] = 4.0
+        ws[2:-1:2] = 2.0
+        ws /= ws.sum()
+    elif rule == "central":
+        xs, ws = np.zeros(1), np.ones(1)
+    else:
+        raise ValueError(rule)
+    for s in range(g.P):
+        Rt = g.rotation_matrix(s).T
+        for c in range(D):
+            phi = 0.5 * (seg_start[c] + seg_end[c]) + 0.5 * (seg_end[c] - seg_start[c]) * xs
+            qs = q_hat(g, phi) @ Rt.T                   # rows: R_s^T q(phi)
+            for i, (l, m) in enumerate(idx):
+                B[s, i, c] = np.dot(ws, real_sh(l, m, qs))
+    return B
+
+
+def basis_forward(B, proj):
+    """Imod[s,j,k,c] = sum_i B[s][i][c] proj[s,j,k,i]   (Eq. 6, inner sum)."""
+    return np.einsum("sjki,sic->sjkc", np.asarray(proj, dtype=np.float64), np.asarray(B, dtype=np.float64))
+
+
+def basis_adjoint(B, sino):
+    """g[s,j,k,i] = sum_c B[s][i][c] sino[s,j,k,c]   (transpose of Eq. 6's inner sum)."""
+    return np.einsum("sjkc,sic->sjki", np.asarray(sino, dtype=np.float64), np.asarray(B, dtype=np.float64))
+
+
+# ------------------------------------------------------------------------------------------------
+# forward model, adjoint, loss and gradient
+# ------------------------------------------------------------------------------------------------
+def forward(g: Geometry, B, vol, threads=None, chunk=16):
+    """I = A c (Eq. 6-7): John transform of every coefficient channel, then the per-projection basis map."""
+    B = np.asarray(B, dtype=np.float64)
+    K, D = B.shape[1], B.shape[2]
+    out = np.empty((g.P,) + g.det + (D,), dtype=np.float64)
+    for s0 in range(0, g.P, chunk):
+        s1 = min(g.P, s0 + chunk)
+        out[s0:s1] = basis_forward(B[s0:s1], john_forward(g, vol, K, s0, s1, threads))
+    return out
+
+
+def adjoint(g: Geometry, B, sino, form="gather", threads=None):
+    """A^T y = John^T (basis^T y), the exact transpose of `forward`."""
+    return john_adjoint(g, basis_adjoint(B, sino), form=form, threads=threads)
+
+
+def loss_gradient(g: Geometry, B, vol, data, weights=None, form="gather", threads=None):
+    """r = A c - I (Eq. 13); L = 1/2 sum w r^2 (Eq. 9 with a = 2, readings S10/S11); grad = A^T (w r).
+    Returns (L, grad[X][Y][Z][K], wr[P][J][Kd][D])."""
+    r = forward(g, B, vol, threads) - np.asarray(data, dtype=np.float64)
+    w = np.ones_like(r) if weights is None else np.asarray(weights, dtype=np.float64)
+    wr = w * r
+    L = 0.5 * float(np.sum(wr * r))
+    return L, adjoint(g, B, wr, form=form, threads=threads), wr
+
+
+def forward_rays(g: Geometry, B, vol, sjk, threads=None):
+    """I[s,j,k,:] for sampled rays sjk[n][3] -> [n][D]."""
+    B = np.asarray(B, dtype=np.float64)
+    sjk = np.asarray(sjk, dtype=np.int32).reshape(-1, 3)
+    p = john_forward_rays(g, vol, B.shape[1], sjk, threads)
+    return np.einsum("ni,nic->nc", p, B[sjk[:, 0]])
+
+
+def gradient_voxels(g: Geometry, B, vol, data, weights, xyz, threads=None):
+    """grad[x, :] of loss_gradient at sampled voxels xyz[n][3], computed from scratch one voxel at a time:
+    the voxel's column of the John matrix (voxel_taps) names the rays that see it; those rays are traced,
+    mapped, compared with the data, and their weighted residuals brought back through B^T and the column."""
+    B = np.asarray(B, dtype=np.float64)
+    xyz = np.asarray(xyz, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((xyz.shape[0], B.shape[1]), dtype=np.float64)
+    for q, (x, y, z) in enumerate(xyz):
+        taps = voxel_taps(g, x, y, z)
+        if taps.shape[0] == 0:
+            continue
+        sjk = taps[:, :3].astype(np.int32)
+        imod = forward_rays(g, B, vol, sjk, threads)
+        s, j, k = sjk[:, 0], sjk[:, 1], sjk[:, 2]
+        r = imod - np.asarray(data[s, j, k], dtype=np.float64)
+        wr = r if weights is None else r * np.asarray(weights[s, j, k], dtype=np.float64)
+        out[q] = np.einsum("n,nic,nc->i", taps[:, 3], B[s], wr)
+    return out
