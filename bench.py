@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the fused gradient iteration of tensor tomography on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5] [--impl ours|reference]
+
+A step = one pass of the whole hot path (Joseph forward + basis map + residual +
+weighted loss + basis^T + exact adjoint) over one synthetic data set, i.e. one `mm_loss_gradient` call.
+Workload at N=1: BASELINE.json configs[4] ("C5": 256^3 voxels, l_max=8 -> K=45, 360 projections, 256^2 pixels,
+D=8), the configuration the metric is quoted on; inputs (3.2 GB volume) exceed the 126 MB L2, so no flush.
+The path does not shard inside the library (BASELINE.json north_star: one GPU, no collectives): --gpus N runs
+N independent replicas ("replicas only") and reports the aggregate.
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2504_16446_b200 import synth  # noqa: E402
+
+METRIC = "fused gradient iteration throughput (G voxel-channel-projections/s); ms per iteration in ms_per_step"
+UNIT = "G vcp/s"
+
+
+def algorithmic_bytes(cfg):
+    """SURVEY.md §8(d) streaming model, unpadded K, 4 B each: forward streams the volume once per projection
+    (4 B per vcp) + writes the D-channel sinogram; the fused gradient adds the gradient write and the data,
+    weights, wr traffic."""
+    N, K, P = cfg.n_voxels, cfg.K, cfg.P
+    sino = P * cfg.det[0] * cfg.det[1] * cfg.D * 4
+    fwd = P * N * K * 4 + sino
+    fused = P * N * K * 4 + N * K * 4 + 4 * sino
+    return fwd, fused
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.proc, self.index = None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); mx.append(float(t[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, t[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        # idle samples (before the first kernel) pull the median down: keep the upper half
+        sm_load = sorted(sm)[len(sm) // 2:] if sm else []
+        return {"sm_mhz": statistics.median(sm_load) if sm_load else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# -------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle on a bounded sample
+# -------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, n_sample_proj):
+    """stratified projection subset: full volume, full detector, n_sample_proj of the P projections."""
+    rot, tilt = synth.angles(cfg)
+    idx = np.unique(((np.arange(n_sample_proj) + 0.5) * cfg.P / n_sample_proj).astype(int))
+    return rot[idx], tilt[idx], idx
+
+
+def run_oracle_step(ora, go, B, vol, data, w, K):
+    t0 = time.perf_counter()
+    ora.loss_gradient(go, B, vol, data, w, form="scatter", threads=1)
+    return time.perf_counter() - t0
+
+
+def oracle_setup(cfg, n_sample_proj, vol=None):
+    from oracle import oracle as ora
+    ora.build()
+    rot, tilt, idx = oracle_sample(cfg, n_sample_proj)
+    go = ora.Geometry(cfg.shape, cfg.det, rot, tilt)
+    B = ora.basis_matrix(go, cfg.ell_max, *synth.segments(cfg.D)).astype(np.float32)
+    if vol is None:
+        vol = synth.make_volume(cfg, cfg.K)
+    data = synth.surrogate_model(cfg)[idx]
+    return ora, go, B, vol, data, idx
+
+
+def sample_size_for(cfg):
+    # ~10-30 s of single-core oracle work; measured ~0.5e9 tap-FMAs/s, 6e9 tap-FMAs per projection at C5
+    per_proj = cfg.det[0] * cfg.det[1] * max(cfg.shape) * 4 * cfg.K * 2
+    return int(max(1, min(cfg.P, 0.9e10 // per_proj)))
+
+
+def reference_arm(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_s = sample_size_for(cfg)
+    ora, go, B, vol, data, idx = oracle_setup(cfg, n_s)
+    K = cfg.K
+    for _ in range(args.warmup):
+        run_oracle_step(ora, go, B, vol[..., :K], data, None, K)
+    ts = [run_oracle_step(ora, go, B, vol[..., :K], data, None, K) for _ in range(args.steps)]
+    t = sum(ts) / len(ts)
+    vcp = cfg.n_voxels * K * len(idx)
+    val = vcp / t / 1e9
+    sample = f"{len(idx)} of {cfg.P} projections (indices {idx.tolist()}), full {cfg.shape} volume and {cfg.det} detector"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: {cfg.shape[0]}x{cfg.shape[1]}x{cfg.shape[2]} voxels, l_max={cfg.ell_max} (K={cfg.K}), "
+            f"P={cfg.P}, detector {cfg.det[0]}x{cfg.det[1]}, D={cfg.D}")
+
+
+# -------------------------------------------------------------------------------------------------
+# our arm
+# -------------------------------------------------------------------------------------------------
+def ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2504_16446_b200 import mm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    mm.load()
+
+    K, D, ldk = cfg.K, cfg.D, synth.ldk_for(cfg.K)
+    rot, tilt = synth.angles(cfg)
+    g = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
+    h_B = mm.mm_basis_sh_matrix(g, cfg.ell_max, *synth.segments(D))
+    t0 = time.time()
+    h_vol = torch.from_numpy(synth.make_volume(cfg, ldk)).pin_memory()
+    h_w = None if cfg.weights == "unit" else torch.from_numpy(synth.make_weights(cfg)).pin_memory()
+    gen_s = time.time() - t0
+    vol, B = h_vol.cuda(), torch.from_numpy(h_B).cuda()
+    w = None if h_w is None else h_w.cuda()
+    # data = forward model + Poisson noise (BASELINE.json configs): model from the parity-tested GPU forward
+    model = torch.empty(g.proj_shape(D), device="cuda")
+    mm.mm_forward(g, B, vol, K, model)
+    h_data = torch.from_numpy(synth.poisson_data(model.cpu().numpy(), cfg.counts, cfg.seed)).pin_memory()
+    del model
+    data = h_data.cuda()
+    grad = torch.empty(g.vol_shape(ldk), device="cuda")
+    wr = torch.empty(g.proj_shape(D), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+
+    def step():
+        mm.mm_loss_gradient(g, B, vol, K, data, w, grad, loss, wr)
+        if cfg.gd_iters > 1:
+            mm.mm_axpy(vol, grad, 1e-9)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    evm = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    for e in evm:
+        e.record()                       # creates the handle the library re-records between the two phases
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = mm.mm_launch_count()
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start.record()
+    for i in range(args.steps):
+        ev0[i].record()
+        mm.mm_set_phase_event(evm[i])
+        step()
+        ev1[i].record()
+    end.record()
+    mm.mm_set_phase_event(None)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = mm.mm_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = start.elapsed_time(end)
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = t.item()
+    ms_step = total_ms / args.steps
+    fwd_ms = sum(a.elapsed_time(b) for a, b in zip(ev0, evm)) / args.steps
+    adj_ms = sum(a.elapsed_time(b) for a, b in zip(evm, ev1)) / args.steps
+    value = world * cfg.vcp / (ms_step * 1e-3) / 1e9
+    loss_val = loss.item()
+
+    # ---- end to end through the host-buffer C-ABI call (H2D of every input, D2H of gradient + loss, inside)
+    e2e = None
+    if rank == 0:
+        h_grad = torch.empty(g.vol_shape(ldk), dtype=torch.float32).pin_memory()
+        del grad, wr
+        torch.cuda.empty_cache()
+        n_e2e = max(1, min(args.steps, 2))
+        mm.mm_loss_gradient_host(g, h_B, h_vol, K, h_data, h_w, h_grad)      # warm-up (page-in, allocator)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            Lh = mm.mm_loss_gradient_host(g, h_B, h_vol, K, h_data, h_w, h_grad)
+        te = (time.perf_counter() - t0) / n_e2e
+        nsino = h_data.numel() * 4
+        e2e = {"value": cfg.vcp / te / 1e9, "unit": UNIT, "ms_per_step": te * 1e3,
+               "h2d_bytes_per_step": int(h_vol.numel() * 4 + nsino * (2 if h_w is not None else 1) + h_B.size * 4),
+               "d2h_bytes_per_step": int(h_grad.numel() * 4 + 8), "steps": n_e2e,
+               "loss_matches_device_path": bool(abs(Lh - loss_val) <= 1e-9 * abs(loss_val)) if cfg.gd_iters <= 1 else None}
+    if rank != 0:
+        return
+
+    peak, peak_src = measured_peaks()
+    fwd_bytes, fused_bytes = algorithmic_bytes(cfg)
+    achieved = fwd_bytes / (fwd_ms * 1e-3) / 1e9
+    roofline = {"kernel": "john_forward_kernel (phase 1 of mm_loss_gradient: Joseph march + basis + residual + loss)",
+                "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "ms_per_launch": fwd_ms,
+                "algorithmic_bytes_per_launch": fwd_bytes,
+                "model": "streaming: 4 B per voxel-channel-projection + sinogram write (SURVEY.md 8d)",
+                "fused_step": {"algorithmic_bytes": fused_bytes, "achieved": fused_bytes / (ms_step * 1e-3) / 1e9,
+                               "frac": fused_bytes / (ms_step * 1e-3) / 1e9 / peak},
+                "adjoint_kernel_ms": adj_ms}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            roofline["traffic"] = json.load(f).get(cfg.name, {}).get("john_forward_kernel_dram_bytes")
+
+    # ---- cpu_baseline: the oracle, single core, on a bounded projection sample of the same workload
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s = sample_size_for(cfg)
+        vol_np = h_vol.numpy()
+        ora, go, Bo, _, data_s, idx = oracle_setup(cfg, n_s, vol=vol_np)
+        t = run_oracle_step(ora, go, Bo, vol_np[..., :K], data_s, None, K)
+        cpu = {"value": cfg.n_voxels * K * len(idx) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "seconds": t, "sample": f"{len(idx)} of {cfg.P} projections (indices {idx.tolist()}), full volume and detector",
+               "host_cores_available": len(os.sched_getaffinity(0))}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "ldk": ldk, "l2": "inputs (%.1f GB volume) larger than L2; no flush" % (vol.numel() * 4 / 1e9),
+                       "multi_gpu": "replicas only", "input_generation_s": round(gen_s, 1)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "loss": loss_val, "phase_ms": {"forward_residual": fwd_ms, "adjoint": adj_ms}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C5", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = synth.get_config(args.config)
+    if args.impl == "reference":
+        reference_arm(args, cfg)
+    else:
+        ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,161 @@
+/* include/mm.h — C ABI of the B200-native tensor-tomography gradient path (arxiv 2504.16446, "Mumott").
+ *
+ * Citations: P:NN = /root/reference/PAPER.md line NN.  Sx = reading x in DESIGN.md "Readings of the paper".
+ *
+ * What the library computes.  A sample is a grid of X*Y*Z voxels, each holding K basis coefficients
+ * c[x][y][z][i] (Eq. 2).  For each of P goniometer settings s (rotation alpha_s, tilt beta_s,
+ * R_s = R_beta R_alpha) and each raster position (j,k) of a J x Kd scan, the forward model is (Eq. 6)
+ *
+ *     I[s][j][k][c] = sum_xyz P_{sjk,xyz} sum_i B[s][i][c] c[x][y][z][i]
+ *
+ * where P_{sjk,xyz} is the John transform (Eq. 5) evaluated by Joseph's method with bilinear
+ * interpolation of the field and B[s][i][c] is the segment-integrated basis matrix of Eq. 3.
+ * The data term of Eq. 9 with residual r = Ac - I (Eq. 13) is L = 1/2 sum w r^2 (S10) and its
+ * gradient is A^T (w r), A^T being the exact transpose of the discrete forward operator (S9).
+ *
+ * Conventions common to every call
+ *   - All functions return mm_status and never throw.  mm_last_error() gives a thread-local message.
+ *   - Arrays are dense, C order, fp32 unless stated.  Layouts:
+ *       volume / gradient   [X][Y][Z][ldk]        channel stride ldk >= K floats ("c[x,y,z,i]")
+ *       K-channel projection [P][J][Kd][ldk]
+ *       sinogram, data, weights, wr  [P][J][Kd][D] (Table IV: data (n_j,n_k,n_phi) per projection)
+ *       basis matrix B      [P][K][D]             (S3)
+ *     Channels K..ldk-1 of INPUT arrays are ignored; of OUTPUT arrays they are written as 0.
+ *   - "DEVICE" pointers are CUDA device memory on the current device, owned by the caller, not aliased with
+ *     each other; the fast path needs ldk % 4 == 0 and 16-byte aligned bases, otherwise a slower scalar path
+ *     runs (same results).  "HOST" pointers are ordinary host memory.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device calls only enqueue
+ *     work on it: no hidden allocation, no synchronisation, outputs overwritten (never accumulated).
+ *   - mm_geometry is immutable after creation; calls on different streams may run concurrently.
+ *   - Errors: NULL required pointer -> MM_ERR_NULL; K<1, ldk<K, D<1, D>MM_MAX_D, shape<1 -> MM_ERR_SHAPE;
+ *     non-finite angle, non-orthonormal axes -> MM_ERR_VALUE; CUDA launch/alloc failures -> MM_ERR_CUDA /
+ *     MM_ERR_ALLOC.  No CPU fallback exists anywhere in this library.
+ */
+#ifndef MM_H_
+#define MM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MM_MAX_D 32          /* most detector segments the kernels hold in registers */
+
+typedef enum {
+    MM_OK = 0,
+    MM_ERR_NULL = 1,
+    MM_ERR_SHAPE = 2,
+    MM_ERR_VALUE = 3,
+    MM_ERR_ALLOC = 4,
+    MM_ERR_CUDA = 5,
+    MM_ERR_UNSUPPORTED = 6
+} mm_status;
+
+typedef struct mm_geometry mm_geometry;      /* opaque */
+
+/* Acquisition geometry (Table I, Table IV, Eq. 4).  HOST memory, borrowed for
+ * the duration of mm_geometry_create only.  A direction given as (0,0,0) takes its Table I standard value. */
+typedef struct {
+    int32_t volume_shape[3];     /* X, Y, Z  (Table IV volume_shape)                                        */
+    int32_t det_shape[2];        /* J, Kd    (raster points along j and k)                                  */
+    int32_t n_proj;              /* P                                                                       */
+    const double *rotations;     /* [P] inner angle alpha_s, radians                                        */
+    const double *tilts;         /* [P] outer angle beta_s, radians                                         */
+    const double *j_offsets;     /* [P] delta j_s in raster steps (Eq. 4), NULL = 0                         */
+    const double *k_offsets;     /* [P] delta k_s, NULL = 0                                                 */
+    double p_dir[3];             /* beam direction p,           standard +z                                 */
+    double j_dir[3];             /* raster direction j,         standard +y (S1)                            */
+    double k_dir[3];             /* raster direction k,         standard +x (S1)                            */
+    double q0_dir[3];            /* detector direction phi=0,   standard +x  (basis helper only)            */
+    double q90_dir[3];           /* detector direction phi=90,  standard +y  (basis helper only)            */
+    double inner_axis[3];        /* rotation axis alpha-hat,    standard +y                                 */
+    double outer_axis[3];        /* tilt axis beta-hat,         standard +x                                 */
+    double voxel_size;           /* a of Eq. 4, 0 = 1                                                       */
+    double pixel_size;           /* b of Eq. 4, 0 = 1                                                       */
+} mm_geometry_desc;
+
+/* Build the per-projection ray table (host, fp64) and upload it to the current CUDA device.  For each s:
+ * d_s = R_s^T p, j_s = R_s^T j, k_s = R_s^T k (sample frame); Joseph major axis m_s = lowest
+ * index with |d_i| >= max|d| - 1e-6 (S8); step w_s = a/|d_m| (S7); the affine maps (j,k,n) -> in-slab position
+ * and voxel -> detector position that follow from Eq. 4 with rotation centre (shape-1)/2 and detector centre
+ * (det-1)/2 (S4).  The library owns *out; free with mm_geometry_destroy. */
+mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometry **out);
+mm_status mm_geometry_destroy(mm_geometry *g);
+
+/* Test introspection: sample-frame beam direction d, raster axes js, ks, major axis and Joseph step of
+ * projection s (all HOST outputs; any may be NULL). */
+mm_status mm_geometry_get(const mm_geometry *g, int32_t s, double d[3], double js[3], double ks[3],
+                          int32_t *major_axis, double *step);
+
+/* HOST helper, Eq. 3 for real spherical harmonics of even degree l <= ell_max,
+ * 4pi-normalised, order l ascending then m = -l..l (S14), small-angle q(phi) = cos(phi) q0 + sin(phi) q90
+ * (Eq. 1 second line): h_B[s][i][c] = mean over [seg_start[c], seg_end[c]] of
+ * Y_i(R_s^T q(phi)), integrated exactly (the integrand is a trigonometric polynomial of degree <= ell_max, S15).
+ * K = (ell_max+1)(ell_max+2)/2.  seg_start/seg_end: [D] radians, HOST.  h_B: [P][K][D] fp32, HOST, caller-owned. */
+mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, int32_t D, const double *seg_start,
+                             const double *seg_end, float *h_B);
+
+/* John transform, Eq. 5 / P:314, ray-stationary Joseph: for every ray (s,j,k) and channel i < K
+ *   proj[s][j][k][i] = w_s * sum_{n=0}^{N_m-1} bilinear(vol[slab n])(pu_n, pv_n)_i, zero outside the volume.
+ * vol [X][Y][Z][ldk] DEVICE in; proj [P][J][Kd][ldk] DEVICE out. */
+mm_status mm_john_forward(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *proj,
+                          void *stream);
+
+/* Exact transpose of mm_john_forward (S9), voxel-stationary gather:
+ *   vol_out[x][i] = sum_s w_s sum_{(j,k)} Lambda(pu(s,j,k;x_m) - x_u) Lambda(pv - x_v) proj[s][j][k][i].
+ * proj [P][J][Kd][ldk] DEVICE in; vol_out [X][Y][Z][ldk] DEVICE out (overwritten). */
+mm_status mm_john_adjoint(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out,
+                          void *stream);
+
+/* Reciprocal-space map of Eq. 6 (inner sum) and its transpose, per pixel:
+ *   forward: sino[s][j][k][c] = sum_i B[s][i][c] proj[s][j][k][i]
+ *   adjoint: proj[s][j][k][i] = sum_c B[s][i][c] sino[s][j][k][c]
+ * B [P][K][D] DEVICE; proj [P][J][Kd][ldk] DEVICE; sino [P][J][Kd][D] DEVICE. */
+mm_status mm_basis_forward(const mm_geometry *g, const float *B, const float *proj, int32_t K, int32_t ldk,
+                           int32_t D, float *sino, void *stream);
+mm_status mm_basis_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk,
+                           int32_t D, float *proj, void *stream);
+
+/* Full forward model I = A c (Eq. 6-7) and its transpose, fused: the K-channel projections stay in
+ * registers and never touch HBM (cf. the paper's fused kernel).
+ *   mm_forward: vol -> sino [P][J][Kd][D];   mm_adjoint: sino -> vol_out [X][Y][Z][ldk] (overwritten). */
+mm_status mm_forward(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                     float *sino, void *stream);
+mm_status mm_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,
+                     float *vol_out, void *stream);
+
+/* One fused gradient evaluation (Eq. 9 data term with a = 2, Eq. 13; S10, S11):
+ *   phase 1 (all rays):   r = (A vol) - data;  wr = weights * r;  *loss = 1/2 sum weights r^2
+ *   phase 2 (all voxels): grad = A^T wr
+ * data, weights [P][J][Kd][D] DEVICE in (weights NULL = all ones); grad [X][Y][Z][ldk] DEVICE out;
+ * loss: DEVICE double, overwritten; wr_workspace [P][J][Kd][D] DEVICE scratch, holds wr on return. */
+mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk,
+                           int32_t D, const float *data, const float *weights, float *grad, double *loss,
+                           float *wr_workspace, void *stream);
+
+/* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */
+mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream);
+
+/* End-to-end convenience with HOST buffers (what a caller without device memory uses): allocates device
+ * buffers, copies B, vol, data, weights host->device, runs mm_loss_gradient, copies grad and loss back,
+ * frees, and synchronises.  All pointers HOST; h_weights may be NULL; h_loss is one double. */
+mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K,
+                                int32_t ldk, int32_t D, const float *h_data, const float *h_weights,
+                                float *h_grad, double *h_loss);
+
+/* Number of kernel launches this library has enqueued since load (for bench accounting). */
+int64_t mm_launch_count(void);
+
+/* Measurement hook: if `cuda_event` (a cudaEvent_t passed as void*) is non-NULL, later mm_loss_gradient calls
+ * made by this host thread record it on their stream between phase 1 and phase 2, so a caller can time the
+ * two kernels of one call separately.  NULL clears the hook.  Does not change what is computed. */
+mm_status mm_set_phase_event(void *cuda_event);
+
+const char *mm_status_string(mm_status s);
+const char *mm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_H_ */

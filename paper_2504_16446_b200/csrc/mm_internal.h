@@ -1,0 +1,53 @@
+// mm_internal.h — private to the CUDA library (never included by oracle/).
+#pragma once
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "mm.h"
+
+// Per-projection ray table entry, built on the host in fp64 (mm_geometry.cpp), read by every kernel.
+//
+// Forward (ray-stationary Joseph; Eq. 4): ray (j,k) of projection s crosses
+// slab n of the major axis m at in-slab position
+//     pu = Cu + j*Mju + k*Mku + n*su,      pv = Cv + j*Mjv + k*Mkv + n*sv         (voxel units)
+// The kernels evaluate this in 32.32 fixed point (exact incremental adds along the ray), hence the *_fx
+// copies of the slopes.
+//
+// Adjoint (voxel-stationary gather): voxel (x,y,z) projects to detector position
+//     j0 = Jc + Jx.x,   k0 = Kc + Kx.x
+// and a ray displaced by (dj,dk) from there passes the voxel's slab at in-slab displacement
+//     du = Mju*dj + Mku*dk,   dv = Mjv*dj + Mkv*dk;   weight = w * Lambda(du) * Lambda(dv).
+// Non-zero weights need |dj| < hj, |dk| < hk (bounding box of M^-1 (-1,1)^2).
+struct MMProj {
+    double Cu, Mju, Mku, su;
+    double Cv, Mjv, Mkv, sv;
+    double Jc, Jx[3];
+    double Kc, Kx[3];
+    long long su_fx, sv_fx;        // round(su * 2^32), round(sv * 2^32)
+    float mju, mku, mjv, mkv;      // fp32 copies for the adjoint weights
+    float hj, hk;                  // candidate window half-widths
+    float w;                       // Joseph step a/|d_m|
+    int m, u, v;                   // major axis and the two in-slab axes (u < v)
+};
+
+struct MMProjHost {
+    double R[9];                   // R_s, sample -> lab
+    double d[3], js[3], ks[3];     // sample-frame beam direction and raster axes
+    int m;
+    double w;
+};
+
+struct mm_geometry {
+    int32_t shape[3];
+    int32_t J, Kd, P;
+    double a, b;
+    double q0[3], q90[3];
+    std::vector<MMProjHost> host;
+    std::vector<MMProj> table;
+    MMProj *d_table;               // device copy of `table`
+    int device;
+};
+
+void mm_set_error(const std::string &msg);

@@ -1,0 +1,739 @@
+// mm_kernels.cu — CUDA kernels (sm_100a) and C-ABI entry points of the tensor-tomography gradient path.
+// Citations: P:NN = PAPER.md line NN; Sx = DESIGN.md reading x.  See include/mm.h for the contract.
+//
+// Kernel inventory
+//   john_forward_kernel<VEC,G,NQ,DMAX,MODE>  ray-stationary Joseph march, lanes over channels;
+//        MODE 0: write K-channel projections; MODE 1: fused basis map -> sinogram (Eq. 6);
+//        MODE 2: fused basis map + residual + weighted loss (Eq. 13, Eq. 9) -> wr, loss
+//   john_adjoint_kernel<VEC,G,NQ>            exact-transpose voxel gather of K-channel projections (S9)
+//   adjoint_fused_kernel<KMAX,DMAX>          voxel gather of the D-channel sinogram, then B^T (Eq. 6 transposed)
+//   basis_forward_kernel / basis_adjoint_kernel, axpy_kernel
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <string>
+
+#include "mm_internal.h"
+
+static std::atomic<long long> g_launches{0};
+
+extern "C" int64_t mm_launch_count(void) { return (int64_t)g_launches.load(); }
+
+static thread_local cudaEvent_t g_phase_event = nullptr;
+
+extern "C" mm_status mm_set_phase_event(void *cuda_event)
+{
+    g_phase_event = (cudaEvent_t)cuda_event;
+    return MM_OK;
+}
+
+#define FX_ONE 4294967296.0            // 2^32
+#define FX_INV 2.3283064365386963e-10f // 2^-32
+
+// ================================================================================================
+// forward: ray-stationary Joseph
+// ================================================================================================
+struct FwdArgs {
+    const MMProj *tab;
+    const float *vol;
+    int K, ldk;
+    int X, Y, Z, J, Kd, P;
+    float *proj;              // MODE 0 out [P][J][Kd][ldk]
+    const float *B;           // MODE 1,2 [P][K][D]
+    int D;
+    const float *data;        // MODE 2
+    const float *weights;     // MODE 2 (may be NULL)
+    float *sino;              // MODE 1: model sinogram; MODE 2: wr
+    double *loss;             // MODE 2
+};
+
+template <int VEC>
+struct Ld;
+template <>
+struct Ld<4> {
+    static __device__ __forceinline__ void ld(const float *p, float (&v)[4])
+    {
+        const float4 t = __ldg(reinterpret_cast<const float4 *>(p));
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    }
+    static __device__ __forceinline__ void st(float *p, const float (&v)[4])
+    {
+        *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    }
+};
+template <>
+struct Ld<1> {
+    static __device__ __forceinline__ void ld(const float *p, float (&v)[1]) { v[0] = __ldg(p); }
+    static __device__ __forceinline__ void st(float *p, const float (&v)[1]) { *p = v[0]; }
+};
+
+// keep the slabs n in [lo,hi] on which -1 < A + n*s < N can hold (one slab of slack on each side)
+__device__ __forceinline__ void clip_range(double A, double s, int N, double &lo, double &hi)
+{
+    if (fabs(s) < 1e-12) {
+        if (!(A > -1.0 && A < (double)N)) hi = lo - 1.0;
+        return;
+    }
+    double t0 = (-1.0 - A) / s, t1 = ((double)N - A) / s;
+    if (t0 > t1) { const double t = t0; t0 = t1; t1 = t; }
+    lo = fmax(lo, t0 - 1.0);
+    hi = fmin(hi, t1 + 1.0);
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Tile of rays per block: TK rays along k (fastest), RPB/TK along j.
+template <int VEC, int G, int NQ, int DMAX, int MODE>
+__global__ void __launch_bounds__(256) john_forward_kernel(const FwdArgs a)
+{
+    constexpr int RPB = 256 / G;                  // rays per block
+    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
+    constexpr int TJ = RPB / TK;
+    const int tid = threadIdx.x;
+    const int q = tid % G;                        // lane within the ray's group
+    const int r = tid / G;                        // ray within the block
+    const int tiles_k = (a.Kd + TK - 1) / TK, tiles_j = (a.J + TJ - 1) / TJ;
+    int tile = blockIdx.x;
+    const int tk = tile % tiles_k; tile /= tiles_k;
+    const int tj = tile % tiles_j;
+    const int s = tile / tiles_j;
+    const int j = tj * TJ + r / TK, k = tk * TK + r % TK;
+    const bool ray_ok = (j < a.J) && (k < a.Kd);
+
+    const MMProj *pg = a.tab + s;
+    const int m = pg->m, u = pg->u, v = pg->v;
+    // (m,u,v) is one of (0,1,2), (1,0,2), (2,0,1)
+    const int Nm = (m == 0) ? a.X : (m == 1 ? a.Y : a.Z);
+    const int Nu = (u == 0) ? a.X : a.Y, Nv = (v == 2) ? a.Z : a.Y;
+    const long long sX = (long long)a.Y * a.Z * a.ldk, sY = (long long)a.Z * a.ldk, sZ = a.ldk;
+    const long long sM = (m == 0) ? sX : (m == 1 ? sY : sZ);
+    const long long sU = (u == 0) ? sX : sY, sV = (v == 2) ? sZ : sY;
+
+    float acc[NQ][VEC];
+#pragma unroll
+    for (int t = 0; t < NQ; t++)
+#pragma unroll
+        for (int x = 0; x < VEC; x++) acc[t][x] = 0.f;
+
+    if (ray_ok) {
+        const double Au = pg->Cu + (double)j * pg->Mju + (double)k * pg->Mku;
+        const double Av = pg->Cv + (double)j * pg->Mjv + (double)k * pg->Mkv;
+        double lo = 0.0, hi = (double)(Nm - 1);
+        clip_range(Au, pg->su, Nu, lo, hi);
+        clip_range(Av, pg->sv, Nv, lo, hi);
+        const int n0 = (int)ceil(lo), n1 = (int)floor(hi);
+        const long long su_fx = pg->su_fx, sv_fx = pg->sv_fx;
+        // 32.32 fixed point: the integer part is the tap index, the fraction the bilinear weight
+        long long pu = (long long)floor(Au * FX_ONE) + (long long)n0 * su_fx;
+        long long pv = (long long)floor(Av * FX_ONE) + (long long)n0 * sv_fx;
+        const float *slab = a.vol + (long long)n0 * sM;
+        for (int n = n0; n <= n1; n++) {
+            const int iu = (int)(pu >> 32), iv = (int)(pv >> 32);
+            const float fu = (float)(unsigned int)(pu & 0xffffffffLL) * FX_INV;
+            const float fv = (float)(unsigned int)(pv & 0xffffffffLL) * FX_INV;
+            const bool u0 = (unsigned)iu < (unsigned)Nu, u1 = (unsigned)(iu + 1) < (unsigned)Nu;
+            const bool v0 = (unsigned)iv < (unsigned)Nv, v1 = (unsigned)(iv + 1) < (unsigned)Nv;
+            const float w00 = (1.f - fu) * (1.f - fv), w10 = fu * (1.f - fv), w01 = (1.f - fu) * fv, w11 = fu * fv;
+            const float *p00 = slab + (long long)iu * sU + (long long)iv * sV;
+#pragma unroll
+            for (int t = 0; t < NQ; t++) {
+                const int e = q + G * t;
+                if (VEC * e < a.ldk) {
+                    float c00[VEC], c10[VEC], c01[VEC], c11[VEC];
+#pragma unroll
+                    for (int x = 0; x < VEC; x++) c00[x] = c10[x] = c01[x] = c11[x] = 0.f;
+                    const float *pe = p00 + VEC * e;
+                    if (u0 && v0) Ld<VEC>::ld(pe, c00);
+                    if (u1 && v0) Ld<VEC>::ld(pe + sU, c10);
+                    if (u0 && v1) Ld<VEC>::ld(pe + sV, c01);
+                    if (u1 && v1) Ld<VEC>::ld(pe + sU + sV, c11);
+#pragma unroll
+                    for (int x = 0; x < VEC; x++) {
+                        acc[t][x] = fmaf(w00, c00[x], acc[t][x]);
+                        acc[t][x] = fmaf(w10, c10[x], acc[t][x]);
+                        acc[t][x] = fmaf(w01, c01[x], acc[t][x]);
+                        acc[t][x] = fmaf(w11, c11[x], acc[t][x]);
+                    }
+                }
+            }
+            pu += su_fx; pv += sv_fx; slab += sM;
+        }
+    }
+    const float w = pg->w;
+    const long long ray = ((long long)s * a.J + j) * a.Kd + k;
+
+    if constexpr (MODE == 0) {
+        if (!ray_ok) return;
+#pragma unroll
+        for (int t = 0; t < NQ; t++) {
+            const int e = q + G * t;
+            if (VEC * e < a.ldk) {
+                float o[VEC];
+#pragma unroll
+                for (int x = 0; x < VEC; x++) o[x] = (VEC * e + x < a.K) ? w * acc[t][x] : 0.f;
+                Ld<VEC>::st(a.proj + ray * a.ldk + VEC * e, o);
+            }
+        }
+        return;
+    } else {
+
+    // fused reciprocal-space map (Eq. 6): Imod[c] = sum_i B[s][i][c] p[i], reduced over the ray's G lanes
+    float part[DMAX];
+#pragma unroll
+    for (int c = 0; c < DMAX; c++) part[c] = 0.f;
+    const float *Bs = a.B + (long long)s * a.K * a.D;
+#pragma unroll
+    for (int t = 0; t < NQ; t++) {
+        const int e = q + G * t;
+#pragma unroll
+        for (int x = 0; x < VEC; x++) {
+            const int i = VEC * e + x;
+            if (i < a.K) {
+                const float pv_ = w * acc[t][x];
+#pragma unroll
+                for (int c = 0; c < DMAX; c++)
+                    if (c < a.D) part[c] = fmaf(__ldg(Bs + (long long)i * a.D + c), pv_, part[c]);
+            }
+        }
+    }
+    if constexpr (G > 1) {
+#pragma unroll
+        for (int o = G / 2; o > 0; o >>= 1)
+#pragma unroll
+            for (int c = 0; c < DMAX; c++) part[c] += __shfl_xor_sync(0xffffffffu, part[c], o);
+    }
+
+    double lsum = 0.0;
+#pragma unroll
+    for (int c = 0; c < DMAX; c++) {
+        if ((c % G) == q && c < a.D && ray_ok) {
+            const long long o = ray * a.D + c;
+            if (MODE == 1) {
+                a.sino[o] = part[c];
+            } else {
+                const float res = part[c] - __ldg(a.data + o);            // r = Ac - I  (Eq. 13)
+                const float wt = a.weights ? __ldg(a.weights + o) : 1.f;
+                const float wr = wt * res;
+                a.sino[o] = wr;
+                lsum += 0.5 * (double)wr * (double)res;                    // L = 1/2 sum w r^2  (S10)
+            }
+        }
+    }
+    if (MODE == 2) {
+        __shared__ double red[8];
+        lsum = warp_sum(lsum);
+        if ((tid & 31) == 0) red[tid >> 5] = lsum;
+        __syncthreads();
+        if (tid == 0) {
+            double tot = 0.0;
+#pragma unroll
+            for (int i = 0; i < 8; i++) tot += red[i];
+            if (tot != 0.0) atomicAdd(a.loss, tot);
+        }
+    }
+    }   // MODE != 0
+}
+
+// ================================================================================================
+// adjoint, K-channel (standalone mm_john_adjoint): voxel-stationary gather, lanes over channels
+// ================================================================================================
+struct AdjArgs {
+    const MMProj *tab;
+    const float *src;         // K-channel: proj [P][J][Kd][ldk]; fused: sino [P][J][Kd][D]
+    const float *B;           // fused only
+    float *out;               // [X][Y][Z][ldk]
+    int K, ldk, D;
+    int X, Y, Z, J, Kd, P;
+    int vec_ok;               // fused: D % 4 == 0 and src 16-byte aligned
+};
+
+template <int VEC, int G, int NQ>
+__global__ void __launch_bounds__(256) john_adjoint_kernel(const AdjArgs a)
+{
+    constexpr int VPB = 256 / G;
+    const int tid = threadIdx.x;
+    const int q = tid % G;
+    const long long vox = (long long)blockIdx.x * VPB + tid / G;
+    const long long nvox = (long long)a.X * a.Y * a.Z;
+    if (vox >= nvox) return;
+    const int z = (int)(vox % a.Z), y = (int)((vox / a.Z) % a.Y), x = (int)(vox / ((long long)a.Z * a.Y));
+    float acc[NQ][VEC];
+#pragma unroll
+    for (int t = 0; t < NQ; t++)
+#pragma unroll
+        for (int c = 0; c < VEC; c++) acc[t][c] = 0.f;
+
+    for (int s = 0; s < a.P; s++) {
+        const MMProj *pg = a.tab + s;
+        const double j0 = fma((double)x, pg->Jx[0], fma((double)y, pg->Jx[1], fma((double)z, pg->Jx[2], pg->Jc)));
+        const double k0 = fma((double)x, pg->Kx[0], fma((double)y, pg->Kx[1], fma((double)z, pg->Kx[2], pg->Kc)));
+        const double fj0 = floor(j0), fk0 = floor(k0);
+        const int jb = (int)fj0, kb = (int)fk0;
+        const float fj = (float)(j0 - fj0), fk = (float)(k0 - fk0);
+        const float hj = pg->hj, hk = pg->hk, w = pg->w;
+        const float mju = pg->mju, mku = pg->mku, mjv = pg->mjv, mkv = pg->mkv;
+        const int djlo = max((int)ceilf(fj - hj), -jb), djhi = min((int)floorf(fj + hj), a.J - 1 - jb);
+        const int dklo = max((int)ceilf(fk - hk), -kb), dkhi = min((int)floorf(fk + hk), a.Kd - 1 - kb);
+        for (int dj = djlo; dj <= djhi; dj++) {
+            const float ej = (float)dj - fj;
+            for (int dk = dklo; dk <= dkhi; dk++) {
+                const float ek = (float)dk - fk;
+                const float du = fmaf(mju, ej, mku * ek), dv = fmaf(mjv, ej, mkv * ek);
+                const float wt = w * fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
+                if (wt > 0.f) {
+                    const float *p = a.src + (((long long)s * a.J + (jb + dj)) * a.Kd + (kb + dk)) * a.ldk;
+#pragma unroll
+                    for (int t = 0; t < NQ; t++) {
+                        const int e = q + G * t;
+                        if (VEC * e < a.ldk) {
+                            float c[VEC];
+                            Ld<VEC>::ld(p + VEC * e, c);
+#pragma unroll
+                            for (int xx = 0; xx < VEC; xx++) acc[t][xx] = fmaf(wt, c[xx], acc[t][xx]);
+                        }
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < NQ; t++) {
+        const int e = q + G * t;
+        if (VEC * e < a.ldk) {
+            float o[VEC];
+#pragma unroll
+            for (int xx = 0; xx < VEC; xx++) o[xx] = (VEC * e + xx < a.K) ? acc[t][xx] : 0.f;
+            Ld<VEC>::st(a.out + vox * a.ldk + VEC * e, o);
+        }
+    }
+}
+
+// ================================================================================================
+// adjoint, fused (mm_adjoint, phase 2 of mm_loss_gradient): thread per voxel gathers the D-channel
+// sinogram with the exact-transpose weights, then applies B_s^T; K accumulators live in registers.
+// ================================================================================================
+#define ADJ_PCH 8        // projections staged in shared memory per step
+
+struct AdjProjS {        // the fields of MMProj the gather needs
+    double Jc, Jx0, Jx1, Jx2, Kc, Kx0, Kx1, Kx2;
+    float mju, mku, mjv, mkv, hj, hk, w, pad;
+};
+
+template <int KMAX, int DMAX>
+__global__ void __launch_bounds__(128) adjoint_fused_kernel(const AdjArgs a)
+{
+    __shared__ AdjProjS sp[ADJ_PCH];
+    __shared__ __align__(16) float sB[ADJ_PCH][KMAX * DMAX];
+    const int tid = threadIdx.x;
+    const long long vox = (long long)blockIdx.x * 128 + tid;
+    const long long nvox = (long long)a.X * a.Y * a.Z;
+    const bool ok = vox < nvox;
+    const long long vv = ok ? vox : nvox - 1;
+    const int z = (int)(vv % a.Z), y = (int)((vv / a.Z) % a.Y), x = (int)(vv / ((long long)a.Z * a.Y));
+    const int i0 = blockIdx.y * KMAX;             // channel chunk handled by this block
+    float acc[KMAX];
+#pragma unroll
+    for (int i = 0; i < KMAX; i++) acc[i] = 0.f;
+
+    for (int s0 = 0; s0 < a.P; s0 += ADJ_PCH) {
+        const int ns = min(ADJ_PCH, a.P - s0);
+        __syncthreads();
+        if (tid < ns) {
+            const MMProj *pg = a.tab + s0 + tid;
+            AdjProjS t;
+            t.Jc = pg->Jc; t.Jx0 = pg->Jx[0]; t.Jx1 = pg->Jx[1]; t.Jx2 = pg->Jx[2];
+            t.Kc = pg->Kc; t.Kx0 = pg->Kx[0]; t.Kx1 = pg->Kx[1]; t.Kx2 = pg->Kx[2];
+            t.mju = pg->mju; t.mku = pg->mku; t.mjv = pg->mjv; t.mkv = pg->mkv;
+            t.hj = pg->hj; t.hk = pg->hk; t.w = pg->w; t.pad = 0.f;
+            sp[tid] = t;
+        }
+        for (int idx = tid; idx < ns * KMAX * DMAX; idx += 128) {
+            const int ps = idx / (KMAX * DMAX), rem = idx % (KMAX * DMAX);
+            const int i = i0 + rem / DMAX, c = rem % DMAX;
+            sB[ps][rem] = (i < a.K && c < a.D) ? __ldg(a.B + ((long long)(s0 + ps) * a.K + i) * a.D + c) : 0.f;
+        }
+        __syncthreads();
+        for (int ps = 0; ps < ns; ps++) {
+            const AdjProjS &pg = sp[ps];
+            const int s = s0 + ps;
+            float t[DMAX];
+#pragma unroll
+            for (int c = 0; c < DMAX; c++) t[c] = 0.f;
+            const double j0 = fma((double)x, pg.Jx0, fma((double)y, pg.Jx1, fma((double)z, pg.Jx2, pg.Jc)));
+            const double k0 = fma((double)x, pg.Kx0, fma((double)y, pg.Kx1, fma((double)z, pg.Kx2, pg.Kc)));
+            const double fj0 = floor(j0), fk0 = floor(k0);
+            const int jb = (int)fj0, kb = (int)fk0;
+            const float fj = (float)(j0 - fj0), fk = (float)(k0 - fk0);
+            const int djlo = max((int)ceilf(fj - pg.hj), -jb), djhi = min((int)floorf(fj + pg.hj), a.J - 1 - jb);
+            const int dklo = max((int)ceilf(fk - pg.hk), -kb), dkhi = min((int)floorf(fk + pg.hk), a.Kd - 1 - kb);
+            for (int dj = djlo; dj <= djhi; dj++) {
+                const float ej = (float)dj - fj;
+                for (int dk = dklo; dk <= dkhi; dk++) {
+                    const float ek = (float)dk - fk;
+                    const float du = fmaf(pg.mju, ej, pg.mku * ek), dv = fmaf(pg.mjv, ej, pg.mkv * ek);
+                    const float wt = pg.w * fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
+                    if (wt > 0.f) {
+                        const float *p = a.src + (((long long)s * a.J + (jb + dj)) * a.Kd + (kb + dk)) * a.D;
+                        if (a.vec_ok) {
+#pragma unroll
+                            for (int c = 0; c < DMAX; c += 4) {
+                                if (c < a.D) {
+                                    const float4 r = __ldg(reinterpret_cast<const float4 *>(p + c));
+                                    t[c] = fmaf(wt, r.x, t[c]); t[c + 1] = fmaf(wt, r.y, t[c + 1]);
+                                    t[c + 2] = fmaf(wt, r.z, t[c + 2]); t[c + 3] = fmaf(wt, r.w, t[c + 3]);
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < DMAX; c++)
+                                if (c < a.D) t[c] = fmaf(wt, __ldg(p + c), t[c]);
+                        }
+                    }
+                }
+            }
+            // acc[i] += sum_c B[s][i][c] t[c]   (transpose of Eq. 6's inner sum)
+            const float4 *b4 = reinterpret_cast<const float4 *>(sB[ps]);
+#pragma unroll
+            for (int i = 0; i < KMAX; i++) {
+#pragma unroll
+                for (int c = 0; c < DMAX; c += 4) {
+                    const float4 b = b4[(i * DMAX + c) / 4];
+                    acc[i] = fmaf(b.x, t[c], acc[i]); acc[i] = fmaf(b.y, t[c + 1], acc[i]);
+                    acc[i] = fmaf(b.z, t[c + 2], acc[i]); acc[i] = fmaf(b.w, t[c + 3], acc[i]);
+                }
+            }
+        }
+    }
+    if (!ok) return;
+    float *o = a.out + vox * a.ldk;
+#pragma unroll
+    for (int i = 0; i < KMAX; i++) {
+        const int ch = i0 + i;
+        if (ch < a.ldk) o[ch] = (ch < a.K) ? acc[i] : 0.f;
+    }
+}
+
+// ================================================================================================
+// standalone reciprocal-space maps and the GD update
+// ================================================================================================
+__global__ void basis_forward_kernel(const float *__restrict__ B, const float *__restrict__ proj, float *__restrict__ sino,
+                                     int K, int ldk, int D, long long npix_per_proj, long long total)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // (pixel, c)
+    if (idx >= total) return;
+    const long long pix = idx / D;
+    const int c = (int)(idx % D);
+    const long long s = pix / npix_per_proj;
+    const float *Bs = B + s * K * D + c;
+    const float *p = proj + pix * ldk;
+    float sum = 0.f;
+    for (int i = 0; i < K; i++) sum = fmaf(__ldg(Bs + (long long)i * D), __ldg(p + i), sum);
+    sino[idx] = sum;
+}
+
+__global__ void basis_adjoint_kernel(const float *__restrict__ B, const float *__restrict__ sino, float *__restrict__ proj,
+                                     int K, int ldk, int D, long long npix_per_proj, long long total)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // (pixel, i)
+    if (idx >= total) return;
+    const long long pix = idx / ldk;
+    const int i = (int)(idx % ldk);
+    float sum = 0.f;
+    if (i < K) {
+        const long long s = pix / npix_per_proj;
+        const float *Bs = B + (s * K + i) * D;
+        const float *y = sino + pix * D;
+        for (int c = 0; c < D; c++) sum = fmaf(__ldg(Bs + c), __ldg(y + c), sum);
+    }
+    proj[idx] = sum;
+}
+
+__global__ void axpy_kernel(float *__restrict__ c, const float *__restrict__ g, float eta, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) c[i] = fmaf(-eta, g[i], c[i]);
+}
+
+// ================================================================================================
+// host-side dispatch
+// ================================================================================================
+namespace {
+
+mm_status check_launch(const char *what)
+{
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        mm_set_error(std::string(what) + ": " + cudaGetErrorString(e));
+        return MM_ERR_CUDA;
+    }
+    g_launches.fetch_add(1);
+    return MM_OK;
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+mm_status check_common(const mm_geometry *g, int K, int ldk, const char *who)
+{
+    if (!g) { mm_set_error(std::string(who) + ": NULL geometry"); return MM_ERR_NULL; }
+    if (!g->d_table) { mm_set_error(std::string(who) + ": geometry was created without a CUDA device (no CPU fallback)"); return MM_ERR_CUDA; }
+    if (K < 1 || ldk < K) { mm_set_error(std::string(who) + ": need 1 <= K <= ldk"); return MM_ERR_SHAPE; }
+    if (K > 256) { mm_set_error(std::string(who) + ": K > 256 is not supported"); return MM_ERR_UNSUPPORTED; }
+    return MM_OK;
+}
+
+template <int VEC, int G, int NQ, int DMAX, int MODE>
+void launch_fwd(const FwdArgs &a, cudaStream_t st)
+{
+    constexpr int RPB = 256 / G;
+    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
+    constexpr int TJ = RPB / TK;
+    const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
+    john_forward_kernel<VEC, G, NQ, DMAX, MODE><<<(unsigned)tiles, 256, 0, st>>>(a);
+}
+
+template <int DMAX, int MODE>
+mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
+{
+    if (vec) {
+        const int lpv = a.ldk / 4;
+        if (lpv <= 1) launch_fwd<4, 1, 1, DMAX, MODE>(a, st);
+        else if (lpv <= 2) launch_fwd<4, 2, 1, DMAX, MODE>(a, st);
+        else if (lpv <= 4) launch_fwd<4, 4, 1, DMAX, MODE>(a, st);
+        else if (lpv <= 8) launch_fwd<4, 8, 1, DMAX, MODE>(a, st);
+        else if (lpv <= 16) launch_fwd<4, 16, 1, DMAX, MODE>(a, st);
+        else if (lpv <= 32) launch_fwd<4, 32, 1, DMAX, MODE>(a, st);
+        else launch_fwd<4, 32, 2, DMAX, MODE>(a, st);
+    } else {
+        if (a.ldk <= 32) launch_fwd<1, 32, 1, DMAX, MODE>(a, st);
+        else launch_fwd<1, 32, 8, DMAX, MODE>(a, st);
+    }
+    return check_launch("john_forward_kernel");
+}
+
+template <int MODE>
+mm_status dispatch_fwd_d(const FwdArgs &a, bool vec, cudaStream_t st)
+{
+    if constexpr (MODE == 0) return dispatch_fwd<1, MODE>(a, vec, st);
+    else if (a.D <= 8) return dispatch_fwd<8, MODE>(a, vec, st);
+    if (a.D <= 16) return dispatch_fwd<16, MODE>(a, vec, st);
+    return dispatch_fwd<32, MODE>(a, vec, st);
+}
+
+void fill_fwd(FwdArgs &a, const mm_geometry *g, const float *vol, int K, int ldk)
+{
+    a.tab = g->d_table; a.vol = vol; a.K = K; a.ldk = ldk;
+    a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
+    a.proj = nullptr; a.B = nullptr; a.D = 0; a.data = nullptr; a.weights = nullptr; a.sino = nullptr; a.loss = nullptr;
+}
+
+void fill_adj(AdjArgs &a, const mm_geometry *g, const float *src, const float *B, float *out, int K, int ldk, int D)
+{
+    a.tab = g->d_table; a.src = src; a.B = B; a.out = out; a.K = K; a.ldk = ldk; a.D = D;
+    a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
+    a.vec_ok = 0;
+}
+
+template <int VEC, int G, int NQ>
+void launch_adj(const AdjArgs &a, cudaStream_t st)
+{
+    constexpr int VPB = 256 / G;
+    const long long nvox = (long long)a.X * a.Y * a.Z;
+    john_adjoint_kernel<VEC, G, NQ><<<(unsigned)((nvox + VPB - 1) / VPB), 256, 0, st>>>(a);
+}
+
+template <int KMAX>
+mm_status launch_adj_fused(const AdjArgs &a, cudaStream_t st)
+{
+    const long long nvox = (long long)a.X * a.Y * a.Z;
+    dim3 grid((unsigned)((nvox + 127) / 128), (unsigned)((a.ldk + KMAX - 1) / KMAX));
+    // chunks past K only need to zero the pad channels; they still run the (cheap for them) common path
+    if (a.D <= 8) adjoint_fused_kernel<KMAX, 8><<<grid, 128, 0, st>>>(a);
+    else if (a.D <= 16) adjoint_fused_kernel<KMAX, 16><<<grid, 128, 0, st>>>(a);
+    else if constexpr (KMAX <= 32) adjoint_fused_kernel<KMAX, 32><<<grid, 128, 0, st>>>(a);
+    else { mm_set_error("adjoint_fused_kernel: no instantiation"); return MM_ERR_UNSUPPORTED; }
+    return check_launch("adjoint_fused_kernel");
+}
+
+mm_status run_adjoint_fused(const mm_geometry *g, const float *B, const float *sino, int K, int ldk, int D,
+                            float *out, cudaStream_t st)
+{
+    AdjArgs a;
+    fill_adj(a, g, sino, B, out, K, ldk, D);
+    a.vec_ok = (D % 4 == 0) && aligned16(sino);
+    if (ldk <= 8) return launch_adj_fused<8>(a, st);
+    if (ldk <= 16) return launch_adj_fused<16>(a, st);
+    if (ldk <= 32) return launch_adj_fused<32>(a, st);
+    if (D <= 16) return launch_adj_fused<48>(a, st);
+    return launch_adj_fused<32>(a, st);
+}
+
+}  // namespace
+
+extern "C" mm_status mm_john_forward(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *proj, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_john_forward");
+    if (st != MM_OK) return st;
+    if (!vol || !proj) { mm_set_error("mm_john_forward: NULL buffer"); return MM_ERR_NULL; }
+    FwdArgs a;
+    fill_fwd(a, g, vol, K, ldk);
+    a.proj = proj;
+    const bool vec = (ldk % 4 == 0) && aligned16(vol) && aligned16(proj);
+    return dispatch_fwd_d<0>(a, vec, (cudaStream_t)stream);
+}
+
+extern "C" mm_status mm_forward(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                float *sino, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_forward");
+    if (st != MM_OK) return st;
+    if (!B || !vol || !sino) { mm_set_error("mm_forward: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_forward: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    FwdArgs a;
+    fill_fwd(a, g, vol, K, ldk);
+    a.B = B; a.D = D; a.sino = sino;
+    const bool vec = (ldk % 4 == 0) && aligned16(vol);
+    return dispatch_fwd_d<1>(a, vec, (cudaStream_t)stream);
+}
+
+extern "C" mm_status mm_john_adjoint(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_john_adjoint");
+    if (st != MM_OK) return st;
+    if (!proj || !vol_out) { mm_set_error("mm_john_adjoint: NULL buffer"); return MM_ERR_NULL; }
+    AdjArgs a;
+    fill_adj(a, g, proj, nullptr, vol_out, K, ldk, 0);
+    cudaStream_t cs = (cudaStream_t)stream;
+    if ((ldk % 4 == 0) && aligned16(proj) && aligned16(vol_out)) {
+        const int lpv = ldk / 4;
+        if (lpv <= 1) launch_adj<4, 1, 1>(a, cs);
+        else if (lpv <= 2) launch_adj<4, 2, 1>(a, cs);
+        else if (lpv <= 4) launch_adj<4, 4, 1>(a, cs);
+        else if (lpv <= 8) launch_adj<4, 8, 1>(a, cs);
+        else if (lpv <= 16) launch_adj<4, 16, 1>(a, cs);
+        else if (lpv <= 32) launch_adj<4, 32, 1>(a, cs);
+        else launch_adj<4, 32, 2>(a, cs);
+    } else {
+        if (ldk <= 32) launch_adj<1, 32, 1>(a, cs);
+        else launch_adj<1, 32, 8>(a, cs);
+    }
+    return check_launch("john_adjoint_kernel");
+}
+
+extern "C" mm_status mm_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,
+                                float *vol_out, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_adjoint");
+    if (st != MM_OK) return st;
+    if (!B || !sino || !vol_out) { mm_set_error("mm_adjoint: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_adjoint: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    return run_adjoint_fused(g, B, sino, K, ldk, D, vol_out, (cudaStream_t)stream);
+}
+
+extern "C" mm_status mm_basis_forward(const mm_geometry *g, const float *B, const float *proj, int32_t K, int32_t ldk,
+                                      int32_t D, float *sino, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_basis_forward");
+    if (st != MM_OK) return st;
+    if (!B || !proj || !sino) { mm_set_error("mm_basis_forward: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1) { mm_set_error("mm_basis_forward: D < 1"); return MM_ERR_SHAPE; }
+    const long long npp = (long long)g->J * g->Kd, total = npp * g->P * D;
+    basis_forward_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(B, proj, sino, K, ldk, D, npp, total);
+    return check_launch("basis_forward_kernel");
+}
+
+extern "C" mm_status mm_basis_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk,
+                                      int32_t D, float *proj, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_basis_adjoint");
+    if (st != MM_OK) return st;
+    if (!B || !proj || !sino) { mm_set_error("mm_basis_adjoint: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1) { mm_set_error("mm_basis_adjoint: D < 1"); return MM_ERR_SHAPE; }
+    const long long npp = (long long)g->J * g->Kd, total = npp * g->P * ldk;
+    basis_adjoint_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(B, sino, proj, K, ldk, D, npp, total);
+    return check_launch("basis_adjoint_kernel");
+}
+
+extern "C" mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                      const float *data, const float *weights, float *grad, double *loss,
+                                      float *wr_workspace, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_loss_gradient");
+    if (st != MM_OK) return st;
+    if (!B || !vol || !data || !grad || !loss || !wr_workspace) { mm_set_error("mm_loss_gradient: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_loss_gradient: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    cudaStream_t cs = (cudaStream_t)stream;
+    if (cudaMemsetAsync(loss, 0, sizeof(double), cs) != cudaSuccess) {
+        mm_set_error(std::string("cudaMemsetAsync(loss): ") + cudaGetErrorString(cudaGetLastError()));
+        return MM_ERR_CUDA;
+    }
+    FwdArgs a;
+    fill_fwd(a, g, vol, K, ldk);
+    a.B = B; a.D = D; a.data = data; a.weights = weights; a.sino = wr_workspace; a.loss = loss;
+    const bool vec = (ldk % 4 == 0) && aligned16(vol);
+    st = dispatch_fwd_d<2>(a, vec, cs);                       // phase 1: a3 + a4 + a5
+    if (st != MM_OK) return st;
+    if (g_phase_event && cudaEventRecord(g_phase_event, cs) != cudaSuccess) {
+        mm_set_error(std::string("cudaEventRecord(phase event): ") + cudaGetErrorString(cudaGetLastError()));
+        return MM_ERR_CUDA;
+    }
+    return run_adjoint_fused(g, B, wr_workspace, K, ldk, D, grad, cs);   // phase 2: a6 + a7
+}
+
+extern "C" mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream)
+{
+    if (!c || !grad) { mm_set_error("mm_axpy: NULL buffer"); return MM_ERR_NULL; }
+    if (n < 0) { mm_set_error("mm_axpy: n < 0"); return MM_ERR_SHAPE; }
+    if (n == 0) return MM_OK;
+    axpy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c, grad, eta, (long long)n);
+    return check_launch("axpy_kernel");
+}
+
+extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K, int32_t ldk,
+                                           int32_t D, const float *h_data, const float *h_weights, float *h_grad, double *h_loss)
+{
+    mm_status st = check_common(g, K, ldk, "mm_loss_gradient_host");
+    if (st != MM_OK) return st;
+    if (!h_B || !h_vol || !h_data || !h_grad || !h_loss) { mm_set_error("mm_loss_gradient_host: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_loss_gradient_host: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    const size_t nvol = (size_t)g->shape[0] * g->shape[1] * g->shape[2] * ldk * sizeof(float);
+    const size_t nsino = (size_t)g->P * g->J * g->Kd * D * sizeof(float);
+    const size_t nB = (size_t)g->P * K * D * sizeof(float);
+    float *dB = nullptr, *dvol = nullptr, *ddata = nullptr, *dw = nullptr, *dgrad = nullptr, *dwr = nullptr;
+    double *dloss = nullptr;
+    cudaStream_t cs = nullptr;
+    mm_status rc = MM_OK;
+    cudaError_t e = cudaSuccess;
+#define MM_TRY(call, code)                                                              \
+    if (rc == MM_OK && (e = (call)) != cudaSuccess) {                                    \
+        mm_set_error(std::string(#call) + ": " + cudaGetErrorString(e));                \
+        cudaGetLastError();                                                             \
+        rc = code;                                                                      \
+    }
+    MM_TRY(cudaStreamCreate(&cs), MM_ERR_CUDA);
+    MM_TRY(cudaMalloc((void **)&dB, nB), MM_ERR_ALLOC);
+    MM_TRY(cudaMalloc((void **)&dvol, nvol), MM_ERR_ALLOC);
+    MM_TRY(cudaMalloc((void **)&ddata, nsino), MM_ERR_ALLOC);
+    if (h_weights) MM_TRY(cudaMalloc((void **)&dw, nsino), MM_ERR_ALLOC);
+    MM_TRY(cudaMalloc((void **)&dgrad, nvol), MM_ERR_ALLOC);
+    MM_TRY(cudaMalloc((void **)&dwr, nsino), MM_ERR_ALLOC);
+    MM_TRY(cudaMalloc((void **)&dloss, sizeof(double)), MM_ERR_ALLOC);
+    MM_TRY(cudaMemcpyAsync(dB, h_B, nB, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
+    MM_TRY(cudaMemcpyAsync(dvol, h_vol, nvol, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
+    MM_TRY(cudaMemcpyAsync(ddata, h_data, nsino, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
+    if (h_weights) MM_TRY(cudaMemcpyAsync(dw, h_weights, nsino, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
+    if (rc == MM_OK) rc = mm_loss_gradient(g, dB, dvol, K, ldk, D, ddata, dw, dgrad, dloss, dwr, cs);
+    MM_TRY(cudaMemcpyAsync(h_grad, dgrad, nvol, cudaMemcpyDeviceToHost, cs), MM_ERR_CUDA);
+    MM_TRY(cudaMemcpyAsync(h_loss, dloss, sizeof(double), cudaMemcpyDeviceToHost, cs), MM_ERR_CUDA);
+    MM_TRY(cudaStreamSynchronize(cs), MM_ERR_CUDA);
+#undef MM_TRY
+    cudaFree(dB); cudaFree(dvol); cudaFree(ddata); cudaFree(dw); cudaFree(dgrad); cudaFree(dwr); cudaFree(dloss);
+    if (cs) cudaStreamDestroy(cs);
+    return rc;
+}

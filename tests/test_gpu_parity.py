@@ -1,0 +1,331 @@
+"""GPU parity: every C-ABI device call against the fp64 CPU oracle on the same seeded inputs (run with -m gpu).
+
+Error metric (reading S18, BASELINE.json north_star): E_inf = max|gpu - oracle| / max|oracle| over the
+whole output array <= 1e-5 for projections, sinograms and gradients; |L_gpu - L_ora| / |L_ora| <= 1e-4 for the loss.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2504_16446_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+TOL_LOSS = 1e-4
+
+
+@pytest.fixture(scope="module")
+def mm():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2504_16446_b200 import mm as binding
+    binding.load()           # raises if libmm.so is missing: no fallback
+    return binding
+
+
+def einf(got, want):
+    want = np.asarray(want, dtype=np.float64)
+    got = np.asarray(got, dtype=np.float64)
+    den = np.abs(want).max()
+    return np.abs(got - want).max() / (den if den > 0 else 1.0)
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class Case:
+    """seeded inputs for one geometry, usable by both sides"""
+
+    def __init__(self, shape, det, rot, tilt, K, ldk, D, seed=0, joff=None, koff=None, vecs=None, a=1.0, b=1.0,
+                 vol=None, B=None, weights="uniform"):
+        r = np.random.default_rng(seed)
+        self.shape, self.det, self.K, self.ldk, self.D = tuple(shape), tuple(det), K, ldk, D
+        self.rot, self.tilt = np.asarray(rot, dtype=np.float64), np.asarray(tilt, dtype=np.float64)
+        self.P = self.rot.size
+        self.kw = dict(j_offsets=joff, k_offsets=koff, vecs=vecs, voxel_size=a, pixel_size=b)
+        if vol is None:
+            vol = r.standard_normal(self.shape + (ldk,)).astype(np.float32)
+        self.vol = vol                                               # pad channels hold garbage on purpose
+        self.B = (r.standard_normal((self.P, K, D)).astype(np.float32) if B is None else B)
+        sh = (self.P,) + self.det
+        self.y = r.standard_normal(sh + (ldk,)).astype(np.float32)  # K-channel projections for the adjoint
+        self.sino = r.standard_normal(sh + (D,)).astype(np.float32)
+        self.data = r.standard_normal(sh + (D,)).astype(np.float32)
+        if weights == "uniform":
+            self.w = r.uniform(0.5, 1.5, sh + (D,)).astype(np.float32)
+        elif weights == "mask":
+            self.w = np.ascontiguousarray(np.broadcast_to((r.uniform(size=sh) >= 0.05).astype(np.float32)[..., None], sh + (D,)))
+        else:
+            self.w = None
+
+    def geoms(self, ora, mm):
+        return (ora.Geometry(self.shape, self.det, self.rot, self.tilt, **self.kw),
+                mm.Geometry(self.shape, self.det, self.rot, self.tilt, **self.kw))
+
+
+def cfg_case(name, shape, det, n_rot, seed, joff=False, weights="uniform"):
+    cfg = synth.get_config(name, shape=shape, det=det, n_rot=n_rot)
+    rot, tilt = synth.angles(cfg)
+    ldk = synth.ldk_for(cfg.K)
+    vol = synth.make_volume(cfg, ldk)
+    r = np.random.default_rng(seed)
+    jo = r.uniform(-1.5, 1.5, cfg.P) if joff else None
+    ko = r.uniform(-1.5, 1.5, cfg.P) if joff else None
+    return cfg, Case(cfg.shape, cfg.det, rot, tilt, cfg.K, ldk, cfg.D, seed=seed, joff=jo, koff=ko, vol=vol, weights=weights)
+
+
+def run_all_ops(ora, mm, c, check_fused_composition=True, sh_basis=None):
+    """all device calls on case c vs the oracle; returns dict of errors"""
+    import torch
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = c.B
+    if sh_basis is not None:
+        B = mm.mm_basis_sh_matrix(gm, sh_basis, *synth.segments(D))
+        assert einf(B, ora.basis_matrix(go, sh_basis, *synth.segments(D))) < 1e-6
+    dB, dvol = dev(B), dev(c.vol)
+    errs = {}
+    # --- John forward (a3)
+    proj = torch.full(gm.proj_shape(ldk), float("nan"), device="cuda")
+    mm.mm_john_forward(gm, dvol, K, proj)
+    want = ora.john_forward(go, c.vol, K)
+    got = proj.cpu().numpy()
+    errs["john_forward"] = einf(got[..., :K], want)
+    assert np.all(got[..., K:] == 0.0)                                   # pad channels written as 0
+    # --- John adjoint (a7)
+    dy = dev(c.y)
+    vout = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    mm.mm_john_adjoint(gm, dy, K, vout)
+    want = ora.john_adjoint(go, c.y[..., :K].astype(np.float64), form="scatter")
+    got = vout.cpu().numpy()
+    errs["john_adjoint"] = einf(got[..., :K], want)
+    assert np.all(got[..., K:] == 0.0)
+    # --- basis maps (a4, a6)
+    sino = torch.empty(gm.proj_shape(D), device="cuda")
+    mm.mm_basis_forward(gm, dB, dy, K, sino)
+    errs["basis_forward"] = einf(sino.cpu().numpy(), ora.basis_forward(B, c.y[..., :K]))
+    dsino = dev(c.sino)
+    pr = torch.full(gm.proj_shape(ldk), float("nan"), device="cuda")
+    mm.mm_basis_adjoint(gm, dB, dsino, K, pr)
+    got = pr.cpu().numpy()
+    errs["basis_adjoint"] = einf(got[..., :K], ora.basis_adjoint(B, c.sino))
+    assert np.all(got[..., K:] == 0.0)
+    # --- fused forward model and its transpose
+    model = torch.empty(gm.proj_shape(D), device="cuda")
+    mm.mm_forward(gm, dB, dvol, K, model)
+    want_model = ora.forward(go, B, c.vol[..., :K])
+    errs["forward"] = einf(model.cpu().numpy(), want_model)
+    vout2 = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    mm.mm_adjoint(gm, dB, dsino, K, vout2)
+    want = ora.adjoint(go, B, c.sino, form="scatter")
+    got = vout2.cpu().numpy()
+    errs["adjoint"] = einf(got[..., :K], want)
+    assert np.all(got[..., K:] == 0.0)
+    # --- fused gradient (a8)
+    scale = float(np.abs(want_model).max())
+    data = (want_model + 0.1 * scale * c.data).astype(np.float32)          # data near the model: no giant residuals
+    grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    loss = torch.full((1,), float("nan"), device="cuda", dtype=torch.float64)
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    dw = None if c.w is None else dev(c.w)
+    mm.mm_loss_gradient(gm, dB, dvol, K, dev(data), dw, grad, loss, wr)
+    L, want_grad, want_wr = ora.loss_gradient(go, B, c.vol[..., :K], data, c.w, form="scatter")
+    errs["wr"] = np.abs(wr.cpu().numpy() - want_wr).max() / scale          # residuals cancel: scale by the model
+    got = grad.cpu().numpy()
+    errs["grad"] = einf(got[..., :K], want_grad)
+    errs["loss"] = abs(loss.item() - L) / abs(L)
+    assert np.all(got[..., K:] == 0.0)
+    if check_fused_composition:
+        # fused == composition of the standalone calls, on the GPU
+        mm.mm_john_forward(gm, dvol, K, proj)
+        mm.mm_basis_forward(gm, dB, proj, K, sino)
+        assert einf(sino.cpu().numpy(), model.cpu().numpy()) < 3e-6
+        mm.mm_basis_adjoint(gm, dB, wr, K, pr)
+        mm.mm_john_adjoint(gm, pr, K, vout)
+        assert einf(vout.cpu().numpy()[..., :K], got[..., :K]) < 3e-6
+    return errs
+
+
+def assert_errs(errs):
+    for k, v in errs.items():
+        assert v <= (TOL_LOSS if k == "loss" else TOL), (k, v, errs)
+
+
+def test_c1_full(ora, mm):
+    """BASELINE.json config 1 at full size (32^3, K=6, 60 projections at tilt 0, includes the 45-degree tie)."""
+    cfg, c = cfg_case("C1", None, None, None, seed=1, weights=None)
+    assert_errs(run_all_ops(ora, mm, c, sh_basis=cfg.ell_max))
+
+
+def test_c2_shrunk_masked_ragged(ora, mm):
+    """config 2 recipe (K=15, six tilts, 5% masked pixels) on a ragged grid spanning several tiles."""
+    cfg, c = cfg_case("C2", (40, 36, 44), (45, 50), 6, seed=2, weights="mask")
+    assert_errs(run_all_ops(ora, mm, c, sh_basis=cfg.ell_max))
+
+
+def test_c3_shrunk_offsets(ora, mm):
+    """config 3 recipe (K=45 -> ldk 48, eight tilts up to 45 degrees incl. y-major projections), sub-pixel offsets."""
+    cfg, c = cfg_case("C3", (30, 26, 34), (37, 41), 5, seed=3, joff=True)
+    assert_errs(run_all_ops(ora, mm, c, sh_basis=cfg.ell_max))
+
+
+def test_c4_shrunk_plate(ora, mm):
+    """config 4 recipe (non-cubic plate, K=28, D=16, weights U[0.5,1.5])."""
+    cfg, c = cfg_case("C4", (20, 40, 40), (44, 44), 4, seed=4)
+    assert_errs(run_all_ops(ora, mm, c, sh_basis=cfg.ell_max))
+
+
+def test_c5_shrunk(ora, mm):
+    """config 5 recipe (ellipsoid density, nine tilts) on 48^3."""
+    cfg, c = cfg_case("C5", (48, 48, 48), (48, 48), 4, seed=5, weights=None)
+    assert_errs(run_all_ops(ora, mm, c, sh_basis=cfg.ell_max))
+
+
+@pytest.mark.parametrize("K,ldk,D", [(7, 7, 5), (1, 1, 1), (3, 4, 8), (33, 36, 12), (70, 72, 9), (130, 132, 4), (20, 21, 32)])
+def test_odd_channel_counts(ora, mm, K, ldk, D):
+    """scalar (unaligned ldk) path, K not a multiple of 4, D not a multiple of 4, channel chunking (K > 48)."""
+    r = np.random.default_rng(K)
+    P = 7
+    c = Case((11, 9, 13), (12, 14), r.uniform(0, 2 * math.pi, P), r.uniform(-0.7, 0.7, P), K, ldk, D, seed=K,
+             joff=r.uniform(-1, 1, P), koff=r.uniform(-1, 1, P))
+    assert_errs(run_all_ops(ora, mm, c))
+
+
+def test_rotated_lab_frame_and_size_ratio(ora, mm):
+    """non-standard Table I vectors (voxel gather window wider than in the standard geometry) and a != b."""
+    r = np.random.default_rng(11)
+    P = 9
+    rot, tilt = r.uniform(0, 2 * math.pi, P), r.uniform(-0.6, 0.6, P)
+    s = math.sqrt(0.5)
+    vecs = {"p": (0.0, 0.0, 1.0), "j": (s, s, 0.0), "k": (s, -s, 0.0), "inner_axis": (0.0, 1.0, 0.0), "outer_axis": (1.0, 0.0, 0.0)}
+    assert_errs(run_all_ops(ora, mm, Case((12, 10, 14), (16, 15), rot, tilt, 6, 8, 8, seed=12, vecs=vecs)))
+    assert_errs(run_all_ops(ora, mm, Case((12, 10, 14), (20, 22), rot, tilt, 6, 8, 8, seed=13, a=1.0, b=0.7)))
+    assert_errs(run_all_ops(ora, mm, Case((12, 10, 14), (9, 8), rot, tilt, 6, 8, 8, seed=14, a=0.8, b=1.3)))
+    vecs = {"p": (1.0, 0.0, 0.0), "j": (0.0, 0.0, 1.0), "k": (0.0, 1.0, 0.0), "inner_axis": (0.0, 0.0, 1.0), "outer_axis": (0.0, 1.0, 0.0)}
+    assert_errs(run_all_ops(ora, mm, Case((12, 10, 14), (16, 15), rot, tilt, 6, 8, 8, seed=15, vecs=vecs)))
+
+
+def test_degenerate_shapes(ora, mm):
+    """single voxel, single pixel, single projection, detector much larger / smaller than the sample, thin axes."""
+    for shape, det in [((1, 1, 1), (1, 1)), ((1, 1, 1), (5, 4)), ((6, 1, 5), (3, 9)), ((2, 7, 1), (8, 2)),
+                       ((5, 5, 5), (17, 19)), ((9, 9, 9), (2, 3)), ((1, 8, 8), (8, 8))]:
+        for rot, tilt in [([0.0], [0.0]), ([0.5, math.pi / 4, 2.0], [0.2, 0.0, math.pi / 4])]:
+            c = Case(shape, det, rot, tilt, 4, 4, 8, seed=len(rot) + shape[0])
+            errs = run_all_ops(ora, mm, c)
+            assert_errs(errs)
+
+
+def test_far_offsets_empty_rays(ora, mm):
+    """offsets that push every ray off the sample: all outputs exactly zero, nothing read out of bounds."""
+    import torch
+    c = Case((6, 6, 6), (5, 5), [0.3, 1.0], [0.1, 0.4], 4, 4, 8, seed=3, joff=[100.0, -80.0], koff=[50.0, 60.0])
+    go, gm = c.geoms(ora, mm)
+    proj = torch.full(gm.proj_shape(4), float("nan"), device="cuda")
+    mm.mm_john_forward(gm, dev(c.vol), 4, proj)
+    assert torch.all(proj == 0).item()
+    assert np.all(ora.john_forward(go, c.vol, 4) == 0)
+    vout = torch.full(gm.vol_shape(4), float("nan"), device="cuda")
+    mm.mm_john_adjoint(gm, dev(c.y), 4, vout)
+    assert torch.all(vout == 0).item()
+
+
+def test_gpu_dot_product_identity(mm):
+    """<A x, y> = <x, A^T y> for the GPU pair itself (fused and K-channel), on a multi-tilt geometry with ties."""
+    import torch
+    cfg = synth.get_config("C3", shape=(28, 24, 30), det=(33, 35), n_rot=4)
+    rot, tilt = synth.angles(cfg)
+    r = np.random.default_rng(7)
+    gm = mm.Geometry(cfg.shape, cfg.det, rot, tilt, j_offsets=r.uniform(-1, 1, cfg.P), k_offsets=r.uniform(-1, 1, cfg.P))
+    K, ldk, D = cfg.K, 48, cfg.D
+    x = torch.randn(gm.vol_shape(ldk), device="cuda")
+    x[..., K:] = 0
+    y = torch.randn(gm.proj_shape(ldk), device="cuda")
+    y[..., K:] = 0
+    Ax = torch.empty_like(y)
+    ATy = torch.empty_like(x)
+    mm.mm_john_forward(gm, x, K, Ax)
+    mm.mm_john_adjoint(gm, y, K, ATy)
+    lhs, rhs = (Ax.double() * y.double()).sum().item(), (x.double() * ATy.double()).sum().item()
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs)), (lhs, rhs)
+    B = dev(mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D)))
+    ys = torch.randn(gm.proj_shape(D), device="cuda")
+    Axs = torch.empty_like(ys)
+    mm.mm_forward(gm, B, x, K, Axs)
+    mm.mm_adjoint(gm, B, ys, K, ATy)
+    lhs, rhs = (Axs.double() * ys.double()).sum().item(), (x.double() * ATy.double()).sum().item()
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs)), (lhs, rhs)
+
+
+def test_zero_residual_and_zero_weight(mm):
+    """data = A c gives L ~ 0, grad ~ 0; zero-weight pixels do not contribute (reading S11)."""
+    import torch
+    cfg = synth.get_config("C2", shape=(20, 20, 20), det=(22, 22), n_rot=3)
+    rot, tilt = synth.angles(cfg)
+    gm = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
+    K, ldk, D = cfg.K, 16, cfg.D
+    B = dev(mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D)))
+    vol = dev(synth.make_volume(cfg, ldk))
+    model = torch.empty(gm.proj_shape(D), device="cuda")
+    mm.mm_forward(gm, B, vol, K, model)
+    grad = torch.empty(gm.vol_shape(ldk), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr = torch.empty_like(model)
+    mm.mm_loss_gradient(gm, B, vol, K, model, None, grad, loss, wr)
+    assert loss.item() == 0.0 and torch.all(grad == 0).item()
+    w = (torch.rand(gm.proj_shape(D), device="cuda") > 0.5).float()
+    junk = model + 1e6 * (1 - w) * torch.randn_like(model)               # garbage where the weight is 0
+    mm.mm_loss_gradient(gm, B, vol, K, junk, w, grad, loss, wr)
+    assert loss.item() == 0.0 and torch.all(grad == 0).item()
+
+
+def test_host_entry_point_matches_device_path(ora, mm):
+    import torch
+    cfg, c = cfg_case("C2", (24, 22, 26), (27, 30), 3, seed=9)
+    go, gm = c.geoms(ora, mm)
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(c.D))
+    data = synth.surrogate_model(cfg)
+    h_grad = np.full(gm.vol_shape(c.ldk), np.nan, dtype=np.float32)
+    L = mm.mm_loss_gradient_host(gm, B, c.vol, c.K, data, c.w, h_grad)
+    grad = torch.empty(gm.vol_shape(c.ldk), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr = torch.empty(gm.proj_shape(c.D), device="cuda")
+    mm.mm_loss_gradient(gm, dev(B), dev(c.vol), c.K, dev(data), dev(c.w), grad, loss, wr)
+    assert abs(L - loss.item()) <= 1e-12 * abs(L)
+    assert np.array_equal(h_grad, grad.cpu().numpy())
+    Lo, go_grad, _ = ora.loss_gradient(go, B, c.vol[..., :c.K], data, c.w, form="scatter")
+    assert abs(L - Lo) <= TOL_LOSS * abs(Lo) and einf(h_grad[..., :c.K], go_grad) <= TOL
+
+
+def test_gd_iterations_c4_recipe(ora, mm):
+    """config 4's timed loop (gradient + fixed-step update) on a shrunk plate: trajectory parity."""
+    import torch
+    cfg, c = cfg_case("C4", (12, 24, 24), (26, 26), 3, seed=21)
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    data = synth.poisson_data(ora.forward(go, B, c.vol[..., :K]), cfg.counts, cfg.seed)
+    # eta = 1 / (max w * ||A||_1 ||A||_inf) from |B| and all-ones inputs (DESIGN.md input recipe), oracle side
+    absB = np.abs(B)
+    rows = ora.forward(go, absB, np.ones(c.shape + (K,), np.float32)).max()
+    cols = ora.adjoint(go, absB, np.ones((c.P,) + c.det + (D,)), form="scatter").max()
+    eta = 1.0 / (float(c.w.max()) * rows * cols)
+    x_o = np.zeros(c.shape + (K,), dtype=np.float32)
+    x_g = torch.zeros(gm.vol_shape(ldk), device="cuda")
+    dB, dd, dw = dev(B), dev(data), dev(c.w)
+    grad = torch.empty_like(x_g)
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    for it in range(5):
+        mm.mm_loss_gradient(gm, dB, x_g, K, dd, dw, grad, loss, wr)
+        mm.mm_axpy(x_g, grad, eta)
+        Lo, g_o, _ = ora.loss_gradient(go, B, x_o, data, c.w, form="scatter")
+        if it == 0:
+            assert einf(grad.cpu().numpy()[..., :K], g_o) <= TOL
+        assert abs(loss.item() - Lo) <= TOL_LOSS * abs(Lo)
+        x_o = (x_o.astype(np.float64) - np.float32(eta).astype(np.float64) * g_o).astype(np.float32)
+    assert einf(x_g.cpu().numpy()[..., :K], x_o) <= 1e-4

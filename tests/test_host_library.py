@@ -1,0 +1,138 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/mm.h declares, validates its
+arguments, and its HOST parts (geometry table, SH basis-matrix helper) agree with the independently written
+oracle.  No compute call is made (there is no GPU here); device calls must fail loudly, never fall back."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+
+
+@pytest.fixture(scope="module")
+def mm():
+    from paper_2504_16446_b200 import build, mm as binding
+    build.build()
+    binding.load()
+    return binding
+
+
+def _segs(D):
+    c = np.arange(D)
+    return c * math.pi / D, (c + 1) * math.pi / D
+
+
+def test_exports_every_declared_symbol(mm):
+    hdr = open(os.path.join(ROOT, "include", "mm.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(mm_[a-z0-9_]+)\s*\(", hdr))
+    assert {"mm_geometry_create", "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint",
+            "mm_loss_gradient"} <= declared                      # BASELINE.json north_star's list
+    L = ctypes.CDLL(mm.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == set(mm.SYMBOLS)
+
+
+def test_table1_golden(mm):
+    rows = {}
+    with open(os.path.join(HERE, "golden", "table1_standard_geometry.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            t = line.split()
+            rows[t[0]] = np.array([float(v) for v in t[1:4]])
+    g = mm.Geometry((4, 5, 6), (5, 4), [0.0], [0.0])
+    d, js, ks, m, w = g.get(0)
+    assert np.allclose(d, rows["p"], atol=1e-15) and np.allclose(js, rows["j"], atol=1e-15)
+    assert np.allclose(ks, rows["k"], atol=1e-15)
+    assert m == 2 and w == 1.0
+
+
+def test_geometry_matches_oracle(mm, ora):
+    r = np.random.default_rng(5)
+    P = 40
+    rot = r.uniform(0, 2 * math.pi, P)
+    tilt = r.uniform(-math.pi / 4, math.pi / 4, P)
+    rot[:4] = [math.pi / 4, 0.0, 3 * math.pi / 4, math.pi / 2]             # ties of reading S8
+    tilt[:4] = [0.0, math.pi / 4, 0.3, 0.0]
+    go = ora.Geometry((9, 7, 8), (6, 10), rot, tilt)
+    gm = mm.Geometry((9, 7, 8), (6, 10), rot, tilt)
+    for s in range(P):
+        a, b = go.get(s), gm.get(s)
+        for x, y in zip(a[:3], b[:3]):
+            assert np.abs(x - y).max() < 1e-14
+        assert a[3] == b[3] and abs(a[4] - b[4]) < 1e-13
+    # non-standard (rotated) lab vectors
+    vecs = {"p": (1.0, 0.0, 0.0), "j": (0.0, 0.0, 1.0), "k": (0.0, 1.0, 0.0), "inner_axis": (0.0, 0.0, 1.0),
+            "outer_axis": (0.0, 1.0, 0.0)}
+    go = ora.Geometry((5, 5, 5), (5, 5), rot[:8], tilt[:8], vecs=vecs)
+    gm = mm.Geometry((5, 5, 5), (5, 5), rot[:8], tilt[:8], vecs=vecs)
+    for s in range(8):
+        a, b = go.get(s), gm.get(s)
+        for x, y in zip(a[:3], b[:3]):
+            assert np.abs(x - y).max() < 1e-14
+        assert a[3] == b[3]
+
+
+@pytest.mark.parametrize("ell,D", [(0, 4), (2, 8), (4, 8), (8, 8), (6, 16)])
+def test_sh_matrix_matches_oracle(mm, ora, ell, D):
+    r = np.random.default_rng(ell)
+    P = 12
+    rot, tilt = r.uniform(0, 2 * math.pi, P), r.uniform(0, math.pi / 4, P)
+    rot[0] = tilt[0] = 0.0
+    go = ora.Geometry((4, 4, 4), (4, 4), rot, tilt)
+    gm = mm.Geometry((4, 4, 4), (4, 4), rot, tilt)
+    s0, s1 = _segs(D)
+    Bo = ora.basis_matrix(go, ell, s0, s1, n_quad=48)
+    Bm = mm.mm_basis_sh_matrix(gm, ell, s0, s1)
+    assert Bm.shape == Bo.shape and Bm.dtype == np.float32
+    assert np.abs(Bm - Bo).max() < 4e-7 * max(1.0, np.abs(Bo).max())          # fp32 rounding of the output only
+    assert np.allclose(Bm[:, 0, :], 1.0)                                       # Y_00 = 1 (reading S14)
+    # uneven, partly reversed and zero-width segments
+    s0 = np.array([0.1, 2.0, 0.7, 1.3])
+    s1 = np.array([0.9, 1.1, 0.7 + 1e-15, 4.0])
+    Bo = ora.basis_matrix(go, ell, s0, s1, n_quad=64)
+    Bm = mm.mm_basis_sh_matrix(gm, ell, s0, s1)
+    assert np.abs(Bm - Bo).max() < 4e-7 * max(1.0, np.abs(Bo).max())
+
+
+def test_argument_validation(mm):
+    with pytest.raises(mm.MMError, match="MM_ERR_SHAPE"):
+        mm.Geometry((0, 4, 4), (4, 4), [0.0], [0.0])
+    with pytest.raises(mm.MMError, match="MM_ERR_SHAPE"):
+        mm.Geometry((4, 4, 4), (4, 0), [0.0], [0.0])
+    with pytest.raises(mm.MMError, match="MM_ERR_VALUE"):
+        mm.Geometry((4, 4, 4), (4, 4), [float("nan")], [0.0])
+    with pytest.raises(mm.MMError, match="MM_ERR_VALUE"):
+        mm.Geometry((4, 4, 4), (4, 4), [0.0], [0.0], vecs={"p": (0.0, 0.0, 2.0)})
+    with pytest.raises(mm.MMError, match="MM_ERR_VALUE"):
+        mm.Geometry((4, 4, 4), (4, 4), [0.0], [0.0], vecs={"p": (0.0, 1.0, 0.0)})     # p parallel to j
+    L = mm.load()
+    assert L.mm_geometry_create(None, None) == 1
+    assert L.mm_geometry_destroy(None) == 0
+    g = mm.Geometry((4, 4, 4), (4, 4), [0.0], [0.0])
+    with pytest.raises(mm.MMError, match="MM_ERR_SHAPE"):
+        g.get(3)
+    with pytest.raises(mm.MMError, match="MM_ERR_SHAPE"):
+        mm.mm_basis_sh_matrix(g, 3, *_segs(4))
+    assert L.mm_john_forward(None, None, 1, 1, None, None) == 1
+    assert L.mm_status_string(5) == b"MM_ERR_CUDA"
+
+
+def test_device_calls_fail_loudly_without_gpu(mm):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    g = mm.Geometry((4, 4, 4), (4, 4), [0.0], [0.0])
+    L = mm.load()
+    dummy = ctypes.c_void_p(16)
+    st = L.mm_john_forward(g._h, dummy, 4, 4, dummy, None)
+    assert st == 5 and b"no CPU fallback" in L.mm_last_error()
+    st = L.mm_loss_gradient(g._h, dummy, dummy, 4, 4, 4, dummy, None, dummy, dummy, dummy, None)
+    assert st == 5
+    assert L.mm_launch_count() == 0
