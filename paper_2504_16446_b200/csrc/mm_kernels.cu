@@ -29,6 +29,12 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
     return MM_OK;
 }
 
+#ifndef FWD_MINB
+#define FWD_MINB 4
+#endif
+#ifndef FWD_U
+#define FWD_U 2                         // slabs in flight per lane in the cooperative forward march
+#endif
 #define FX_ONE 4294967296.0            // 2^32
 #define FX_INV 2.3283064365386963e-10f // 2^-32
 
@@ -69,6 +75,14 @@ struct Ld<1> {
     static __device__ __forceinline__ void st(float *p, const float (&v)[1]) { *p = v[0]; }
 };
 
+// read-only 16-byte load that the compiler may not sink below later loads (keeps FWD_U slabs in flight)
+__device__ __forceinline__ float4 ldg_nc_v4(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
 // keep the slabs n in [lo,hi] on which -1 < A + n*s < N can hold (one slab of slack on each side)
 __device__ __forceinline__ void clip_range(double A, double s, int N, double &lo, double &hi)
 {
@@ -89,9 +103,19 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// One slab's four bilinear taps of a ray: offsets from the volume base in float4 units (clamped into the
+// volume) and weights (0 for taps outside the volume: zero padding, S8).
+struct __align__(16) SlabTaps {
+    int o00, o10, o01, o11;
+    float w00, w10, w01, w11;
+};
+
 // Tile of rays per block: TK rays along k (fastest), RPB/TK along j.
-template <int VEC, int G, int NQ, int DMAX, int MODE>
-__global__ void __launch_bounds__(256) john_forward_kernel(const FwdArgs a)
+// COOP (VEC == 4 only): the G lanes of a ray take turns at the index arithmetic — lane q works out the taps of
+// slab nb+q once, parks them in shared memory, and all lanes then stream through G slabs doing nothing but
+// loads and FMAs (v1 spent 21 instructions per LDG.128, profiles/r01_ncu_c5_v1.md).
+template <int VEC, int G, int NQ, int DMAX, int MODE, bool COOP>
+__global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdArgs a)
 {
     constexpr int RPB = 256 / G;                  // rays per block
     constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
@@ -122,7 +146,90 @@ __global__ void __launch_bounds__(256) john_forward_kernel(const FwdArgs a)
 #pragma unroll
         for (int x = 0; x < VEC; x++) acc[t][x] = 0.f;
 
-    if (ray_ok) {
+    if constexpr (COOP) {
+        static_assert(!COOP || VEC == 4, "cooperative march needs float4 lanes");
+        static_assert(G % FWD_U == 0, "a round of G slabs is consumed FWD_U at a time");
+        __shared__ SlabTaps taps[RPB][G];
+        int n0 = 0, n1 = -1;
+        long long pu0 = 0, pv0 = 0;
+        if (ray_ok) {
+            const double Au = pg->Cu + (double)j * pg->Mju + (double)k * pg->Mku;
+            const double Av = pg->Cv + (double)j * pg->Mjv + (double)k * pg->Mkv;
+            double lo = 0.0, hi = (double)(Nm - 1);
+            clip_range(Au, pg->su, Nu, lo, hi);
+            clip_range(Av, pg->sv, Nv, lo, hi);
+            n0 = (int)ceil(lo); n1 = (int)floor(hi);
+            pu0 = (long long)floor(Au * FX_ONE);
+            pv0 = (long long)floor(Av * FX_ONE);
+        }
+        const long long su_fx = pg->su_fx, sv_fx = pg->sv_fx;
+        const int ldk4 = a.ldk >> 2;
+        const int sM4 = (int)(sM >> 2), sU4 = (int)(sU >> 2), sV4 = (int)(sV >> 2);
+        const float4 *vol4 = reinterpret_cast<const float4 *>(a.vol);
+        int rounds = (n1 >= n0) ? (n1 - n0 + G) / G : 0;
+        rounds = __reduce_max_sync(0xffffffffu, rounds);          // the warp's groups step through rounds together
+        for (int rd = 0; rd < rounds; rd++) {
+            const int nb = n0 + rd * G;
+            {   // lane q: taps of slab nb + q
+                const int n = nb + q;
+                SlabTaps t;
+                t.o00 = t.o10 = t.o01 = t.o11 = 0;
+                t.w00 = t.w10 = t.w01 = t.w11 = 0.f;
+                if (n <= n1) {
+                    // 32.32 fixed point: the integer part is the tap index, the fraction the bilinear weight
+                    const long long pu = pu0 + (long long)n * su_fx, pv = pv0 + (long long)n * sv_fx;
+                    const int iu = (int)(pu >> 32), iv = (int)(pv >> 32);
+                    const float fu = (float)(unsigned int)(pu & 0xffffffffLL) * FX_INV;
+                    const float fv = (float)(unsigned int)(pv & 0xffffffffLL) * FX_INV;
+                    const bool u0 = (unsigned)iu < (unsigned)Nu, u1 = (unsigned)(iu + 1) < (unsigned)Nu;
+                    const bool v0 = (unsigned)iv < (unsigned)Nv, v1 = (unsigned)(iv + 1) < (unsigned)Nv;
+                    const int b0 = n * sM4 + (u0 ? iu * sU4 : 0), b1 = n * sM4 + (u1 ? (iu + 1) * sU4 : 0);
+                    const int c0 = v0 ? iv * sV4 : 0, c1 = v1 ? (iv + 1) * sV4 : 0;
+                    t.o00 = b0 + c0; t.o10 = b1 + c0; t.o01 = b0 + c1; t.o11 = b1 + c1;
+                    t.w00 = (u0 && v0) ? (1.f - fu) * (1.f - fv) : 0.f;
+                    t.w10 = (u1 && v0) ? fu * (1.f - fv) : 0.f;
+                    t.w01 = (u0 && v1) ? (1.f - fu) * fv : 0.f;
+                    t.w11 = (u1 && v1) ? fu * fv : 0.f;
+                }
+                taps[r][q] = t;
+            }
+            __syncwarp();
+            // FWD_U slabs per step: all their loads are issued before the first FMA (slabs past n1 carry
+            // zero weights and offset 0, so the tail needs no special case)
+            const int cnt = min(G, n1 - nb + 1);
+            for (int i = 0; i < cnt; i += FWD_U) {
+                int4 o[FWD_U];
+                float4 w[FWD_U];
+#pragma unroll
+                for (int uu = 0; uu < FWD_U; uu++) {
+                    o[uu] = *reinterpret_cast<const int4 *>(&taps[r][i + uu].o00);
+                    w[uu] = *reinterpret_cast<const float4 *>(&taps[r][i + uu].w00);
+                }
+#pragma unroll
+                for (int t = 0; t < NQ; t++) {
+                    // lanes past the last float4 of the voxel re-read its last one (same cache line, result
+                    // discarded in the epilogue): no branch in the loop
+                    const int e = min(q + G * t, ldk4 - 1);
+                    float4 c[FWD_U][4];
+#pragma unroll
+                    for (int uu = 0; uu < FWD_U; uu++) {
+                        c[uu][0] = ldg_nc_v4(vol4 + (o[uu].x + e)); c[uu][1] = ldg_nc_v4(vol4 + (o[uu].y + e));
+                        c[uu][2] = ldg_nc_v4(vol4 + (o[uu].z + e)); c[uu][3] = ldg_nc_v4(vol4 + (o[uu].w + e));
+                    }
+#pragma unroll
+                    for (int uu = 0; uu < FWD_U; uu++) {
+                        const float ww[4] = {w[uu].x, w[uu].y, w[uu].z, w[uu].w};
+#pragma unroll
+                        for (int p = 0; p < 4; p++) {
+                            acc[t][0] = fmaf(ww[p], c[uu][p].x, acc[t][0]); acc[t][1] = fmaf(ww[p], c[uu][p].y, acc[t][1]);
+                            acc[t][2] = fmaf(ww[p], c[uu][p].z, acc[t][2]); acc[t][3] = fmaf(ww[p], c[uu][p].w, acc[t][3]);
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    } else if (ray_ok) {
         const double Au = pg->Cu + (double)j * pg->Mju + (double)k * pg->Mku;
         const double Av = pg->Cv + (double)j * pg->Mjv + (double)k * pg->Mkv;
         double lo = 0.0, hi = (double)(Nm - 1);
@@ -495,7 +602,14 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
     constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
     constexpr int TJ = RPB / TK;
     const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
-    john_forward_kernel<VEC, G, NQ, DMAX, MODE><<<(unsigned)tiles, 256, 0, st>>>(a);
+    if constexpr (VEC == 4 && G >= FWD_U) {
+        // cooperative march: tap offsets are 32-bit float4 indices
+        if ((long long)a.X * a.Y * a.Z * (a.ldk / 4) < (1LL << 31)) {
+            john_forward_kernel<VEC, G, NQ, DMAX, MODE, true><<<(unsigned)tiles, 256, 0, st>>>(a);
+            return;
+        }
+    }
+    john_forward_kernel<VEC, G, NQ, DMAX, MODE, false><<<(unsigned)tiles, 256, 0, st>>>(a);
 }
 
 template <int DMAX, int MODE>
