@@ -51,3 +51,18 @@ struct mm_geometry {
 };
 
 void mm_set_error(const std::string &msg);
+
+// Arguments of the voxel-stationary (adjoint) kernels.
+struct AdjArgs {
+    const MMProj *tab;
+    const float *src;         // K-channel: proj [P][J][Kd][ldk]; fused: sino [P][J][Kd][D]
+    const float *B;           // fused only
+    float *out;               // [X][Y][Z][ldk]
+    int K, ldk, D;
+    int X, Y, Z, J, Kd, P;
+    int vec_ok;               // fused: D % 4 == 0 and src 16-byte aligned
+};
+
+// mm_adjoint_tc.cu: fused adjoint with the basis contraction on the tensor cores (tcgen05, 3xTF32).
+bool mm_adjoint_tc_supported(const AdjArgs &a);
+int mm_adjoint_tc_launch(const AdjArgs &a, void *stream);   // returns a cudaError_t

@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include <atomic>
 #include <string>
@@ -351,16 +352,6 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
 // ================================================================================================
 // adjoint, K-channel (standalone mm_john_adjoint): voxel-stationary gather, lanes over channels
 // ================================================================================================
-struct AdjArgs {
-    const MMProj *tab;
-    const float *src;         // K-channel: proj [P][J][Kd][ldk]; fused: sino [P][J][Kd][D]
-    const float *B;           // fused only
-    float *out;               // [X][Y][Z][ldk]
-    int K, ldk, D;
-    int X, Y, Z, J, Kd, P;
-    int vec_ok;               // fused: D % 4 == 0 and src 16-byte aligned
-};
-
 template <int VEC, int G, int NQ>
 __global__ void __launch_bounds__(256) john_adjoint_kernel(const AdjArgs a)
 {
@@ -681,6 +672,16 @@ mm_status run_adjoint_fused(const mm_geometry *g, const float *B, const float *s
     AdjArgs a;
     fill_adj(a, g, sino, B, out, K, ldk, D);
     a.vec_ok = (D % 4 == 0) && aligned16(sino);
+    static const bool tc_off = getenv("MM_DISABLE_TC") != nullptr;     // debugging switch: CUDA-core contraction
+    if (!tc_off && mm_adjoint_tc_supported(a)) {
+        const cudaError_t e = (cudaError_t)mm_adjoint_tc_launch(a, st);
+        if (e != cudaSuccess) {
+            mm_set_error(std::string("adjoint_tc_kernel: ") + cudaGetErrorString(e));
+            return MM_ERR_CUDA;
+        }
+        g_launches.fetch_add(1);
+        return MM_OK;
+    }
     if (ldk <= 8) return launch_adj_fused<8>(a, st);
     if (ldk <= 16) return launch_adj_fused<16>(a, st);
     if (ldk <= 32) return launch_adj_fused<32>(a, st);

@@ -147,11 +147,12 @@ def run_all_ops(ora, mm, c, check_fused_composition=True, sh_basis=None):
         assert einf(sino.cpu().numpy(), model.cpu().numpy()) < 3e-6
         mm.mm_basis_adjoint(gm, dB, wr, K, pr)
         mm.mm_john_adjoint(gm, pr, K, vout)
-        assert einf(vout.cpu().numpy()[..., :K], got[..., :K]) < 3e-6
+        assert einf(vout.cpu().numpy()[..., :K], got[..., :K]) < 1e-5    # two fp32 paths, each within TOL of the oracle
     return errs
 
 
 def assert_errs(errs):
+    print("parity errors:", {k: float("%.2e" % v) for k, v in errs.items()})
     for k, v in errs.items():
         assert v <= (TOL_LOSS if k == "loss" else TOL), (k, v, errs)
 
