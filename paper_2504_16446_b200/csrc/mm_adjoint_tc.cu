@@ -129,33 +129,26 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const float (&v)[16])
 // random sign); truncating hi instead of rounding it makes lo one-signed and the error a bias (measured).
 __device__ __forceinline__ void split_tf32(float x, float &hi, float &lo)
 {
-    hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+    uint32_t h;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(h) : "f"(x));
+    hi = __uint_as_float(h);
     lo = x - hi;
 }
 
-// the fields of MMProj the voxel gather needs (w_s is folded into the staged B operand)
+// the gather block of MMProj (same 96-byte layout, checked below)
 struct TcProj {
     double Jc, Jx0, Jx1, Jx2, Kc, Kx0, Kx1, Kx2;
-    float mju, mku, mjv, mkv, hj, hk;
-    int valid, pad;
+    float mju, mku, mjv, mkv, hj, hk, w;
+    int valid;                     // MMProj::gcode, or 0 for a projection past the last one
 };
+static_assert(sizeof(TcProj) == 96, "TcProj mirrors the gather block of MMProj");
 
-__device__ __forceinline__ void load_proj(TcProj &t, const MMProj *tab, int s, int P)
+// 12 lanes copy one projection's constants (8 bytes each) from the device table into shared memory
+__device__ __forceinline__ void load_proj(TcProj *dst, const MMProj *tab, int s, int P, int word)
 {
-    if (s < P) {
-        const MMProj *pg = tab + s;
-        t.Jc = pg->Jc; t.Jx0 = pg->Jx[0]; t.Jx1 = pg->Jx[1]; t.Jx2 = pg->Jx[2];
-        t.Kc = pg->Kc; t.Kx0 = pg->Kx[0]; t.Kx1 = pg->Kx[1]; t.Kx2 = pg->Kx[2];
-        t.mju = pg->mju; t.mku = pg->mku; t.mjv = pg->mjv; t.mkv = pg->mkv;
-        t.hj = pg->hj; t.hk = pg->hk;
-        // 1: generic window loop; 4 + 2*(NJ-2) + (NK-2): fixed NJ x NK window
-        t.valid = (pg->hj < 1.5f && pg->hk < 1.5f) ? 4 + 2 * (pg->hj <= 1.00002f ? 0 : 1) + (pg->hk <= 1.00002f ? 0 : 1) : 1;
-    } else {
-        t.Jc = t.Jx0 = t.Jx1 = t.Jx2 = t.Kc = t.Kx0 = t.Kx1 = t.Kx2 = 0.0;
-        t.mju = t.mku = t.mjv = t.mkv = 0.f;
-        t.hj = t.hk = -1.f; t.valid = 0;           // empty candidate window
-    }
-    t.pad = 0;
+    uint2 v = make_uint2(0u, 0u);                  // past the end: all zero, valid = 0
+    if (s < P) v = __ldg(reinterpret_cast<const uint2 *>(&tab[s].Jc) + word);
+    reinterpret_cast<uint2 *>(dst)[word] = v;
 }
 
 // t[c] = sum over the rays (jj,kk) of projection s that pass within one voxel of (x,y,z) in its slab of
@@ -192,6 +185,19 @@ __device__ __forceinline__ void gather_voxel(const TcProj &pg, const float *__re
             }
         }
     }
+}
+
+// v[0..7] = on ? 32 bytes at p : 0 — a predicated read-only 256-bit load (sm_100: LDG.E.256), no branch;
+// p must be 32-byte aligned when on
+__device__ __forceinline__ void ldg256_pred(const void *p, bool on, float *v)
+{
+#pragma unroll
+    for (int i = 0; i < 8; i++) v[i] = 0.f;
+    asm volatile(
+        "{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %9, 0;\n\t"
+        "@q ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7])
+        : "l"(p), "r"((int)on));
 }
 
 // Fast path of gather_voxel for candidate windows NJ x NK rays wide, NJ, NK in {2, 3}: hj <= 1 means at most two
@@ -231,23 +237,26 @@ __device__ __forceinline__ void gather_voxel_fixed(const TcProj &pg, const float
     // 32-bit float4 index into the projection's sinogram (J*Kd*D < 2^31 checked by the host)
     const float4 *src4 = reinterpret_cast<const float4 *>(src_s);
     const int i00 = (jj0 * Kd + kk0) * (D / 4), rstep = Kd * (D / 4);
+    // all candidates' loads are issued (predicated, branch-free) before the first FMA: one memory round trip per
+    // voxel-projection instead of one per candidate
+    float wt[NJ * NK], v[NJ * NK][D];
 #pragma unroll
     for (int r = 0; r < NJ; r++) {
 #pragma unroll
         for (int c = 0; c < NK; c++) {
             const float du = au[r] + bu[c], dv = av[r] + bv[c];
-            const float wt = fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
-            if (wt > 0.f && rok[r] && cok[c]) {
-                const float4 *p = src4 + (i00 + r * rstep + c * (D / 4));
+            const float w = fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
+            const bool on = w > 0.f && rok[r] && cok[c];
+            wt[r * NK + c] = on ? w : 0.f;
+            const float4 *p = src4 + (i00 + r * rstep + c * (D / 4));
 #pragma unroll
-                for (int q = 0; q < D; q += 4) {
-                    const float4 v = __ldg(p + q / 4);
-                    t[q] = fmaf(wt, v.x, t[q]); t[q + 1] = fmaf(wt, v.y, t[q + 1]);
-                    t[q + 2] = fmaf(wt, v.z, t[q + 2]); t[q + 3] = fmaf(wt, v.w, t[q + 3]);
-                }
-            }
+            for (int q = 0; q < D; q += 8) ldg256_pred(p + q / 4, on, &v[r * NK + c][q]);
         }
     }
+#pragma unroll
+    for (int n = 0; n < NJ * NK; n++)
+#pragma unroll
+        for (int i = 0; i < D; i++) t[i] = fmaf(wt[n], v[n][i], t[i]);
 }
 
 // two regions of ACCW columns each: the MMA accumulator of the current window, and the running sum
@@ -313,7 +322,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
                 float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (n < a.K && s < a.P) {
                     b = __ldg(reinterpret_cast<const float4 *>(a.B + ((long long)s * a.K + n) * D + c));
-                    const float w = a.tab[s].w;
+                    const float w = __ldg(&a.tab[s].w);
                     b.x *= w; b.y *= w; b.z *= w; b.w *= w;
                 }
                 float4 h, l;
@@ -385,7 +394,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
         for (int ch = 0; ch < nch; ch++) {
             const int st = ch & 1, s0 = ch * NPC;
             __syncwarp();
-            if (lane < NPC) load_proj(wsp[lane], a.tab, s0 + lane, a.P);     // this warp's copy of the constants
+            if (lane < 12 * NPC) load_proj(wsp + lane / 12, a.tab, s0 + lane / 12, a.P, lane % 12);   // this warp's copy
             __syncwarp();
             if (ch >= 2) mbar_wait(&empty[st], (uint32_t)(((ch >> 1) - 1) & 1));   // MMAs of chunk ch-2 have read stage st
             float *Ahi = sA + (2 * st) * A_FLOATS, *Alo = Ahi + A_FLOATS;
@@ -399,6 +408,10 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
                     case 5: gather_voxel_fixed<D, 2, 3>(pg, src_s, x, y, z, a.J, a.Kd, t); break;
                     case 6: gather_voxel_fixed<D, 3, 2>(pg, src_s, x, y, z, a.J, a.Kd, t); break;
                     case 7: gather_voxel_fixed<D, 3, 3>(pg, src_s, x, y, z, a.J, a.Kd, t); break;
+                    case 0:
+#pragma unroll
+                        for (int c = 0; c < D; c++) t[c] = 0.f;
+                        break;
                     default: gather_voxel<D>(pg, src_s, x, y, z, a.J, a.Kd, t); break;
                 }
 #pragma unroll
@@ -457,7 +470,8 @@ bool mm_adjoint_tc_supported(const AdjArgs &a)
 {
     return a.vec_ok && (a.D == 8 || a.D == 16) && a.ldk % 4 == 0 && a.ldk <= 64 &&
            (long long)a.J * a.Kd * a.D < (1LL << 31) &&
-           (reinterpret_cast<uintptr_t>(a.B) & 15u) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0;
+           (reinterpret_cast<uintptr_t>(a.B) & 15u) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0 &&
+           (reinterpret_cast<uintptr_t>(a.src) & 31u) == 0;      // 256-bit gather loads
 }
 
 int mm_adjoint_tc_launch(const AdjArgs &a, void *stream)

@@ -153,6 +153,9 @@ extern "C" mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometr
         // (dj,dk) = M^-1 (du,dv), |du|,|dv| < 1  =>  |dj| < (|Mkv| + |Mku|)/|det|, |dk| < (|Mjv| + |Mju|)/|det|
         t.hj = (float)((fabs(t.Mkv) + fabs(t.Mku)) / fabs(det) * (1.0 + 1e-6) + 1e-6);
         t.hk = (float)((fabs(t.Mjv) + fabs(t.Mju)) / fabs(det) * (1.0 + 1e-6) + 1e-6);
+        // half-width <= 1: at most 2 candidate rays along that detector axis; < 1.5: at most 3
+        t.gcode = (t.hj < 1.5f && t.hk < 1.5f) ? 4 + 2 * (t.hj <= 1.00002f ? 0 : 1) + (t.hk <= 1.00002f ? 0 : 1) : 1;
+        t.pad_ = 0;
     }
     // Upload the table.  On a machine without a CUDA device the geometry stays host-only (mm_geometry_get and
     // mm_basis_sh_matrix work; every device call then fails with MM_ERR_CUDA — there is no CPU fallback).

@@ -1,5 +1,6 @@
 // mm_internal.h — private to the CUDA library (never included by oracle/).
 #pragma once
+#include <stddef.h>
 #include <stdint.h>
 
 #include <string>
@@ -23,14 +24,19 @@
 struct MMProj {
     double Cu, Mju, Mku, su;
     double Cv, Mjv, Mkv, sv;
+    // --- 96 contiguous bytes read as one block by the tensor-core adjoint (struct TcProj in mm_adjoint_tc.cu) ---
     double Jc, Jx[3];
     double Kc, Kx[3];
-    long long su_fx, sv_fx;        // round(su * 2^32), round(sv * 2^32)
     float mju, mku, mjv, mkv;      // fp32 copies for the adjoint weights
     float hj, hk;                  // candidate window half-widths
     float w;                       // Joseph step a/|d_m|
+    int gcode;                     // gather window: 1 = generic loop; 4 + 2*(NJ-2) + (NK-2) = fixed NJ x NK, NJ,NK in {2,3}
+    // ---
+    long long su_fx, sv_fx;        // round(su * 2^32), round(sv * 2^32)
     int m, u, v;                   // major axis and the two in-slab axes (u < v)
+    int pad_;
 };
+static_assert(offsetof(MMProj, gcode) - offsetof(MMProj, Jc) == 92, "gather block of MMProj must be 96 contiguous bytes");
 
 struct MMProjHost {
     double R[9];                   // R_s, sample -> lab

@@ -243,6 +243,7 @@ def test_gpu_dot_product_identity(mm):
     r = np.random.default_rng(7)
     gm = mm.Geometry(cfg.shape, cfg.det, rot, tilt, j_offsets=r.uniform(-1, 1, cfg.P), k_offsets=r.uniform(-1, 1, cfg.P))
     K, ldk, D = cfg.K, 48, cfg.D
+    torch.manual_seed(7)
     x = torch.randn(gm.vol_shape(ldk), device="cuda")
     x[..., K:] = 0
     y = torch.randn(gm.proj_shape(ldk), device="cuda")
@@ -251,15 +252,16 @@ def test_gpu_dot_product_identity(mm):
     ATy = torch.empty_like(x)
     mm.mm_john_forward(gm, x, K, Ax)
     mm.mm_john_adjoint(gm, y, K, ATy)
+    # white-noise inner products cancel, so the scale of the comparison is |Ax||y| (Cauchy-Schwarz), not |<Ax,y>|
     lhs, rhs = (Ax.double() * y.double()).sum().item(), (x.double() * ATy.double()).sum().item()
-    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs)), (lhs, rhs)
+    assert abs(lhs - rhs) <= 1e-5 * (Ax.double().norm() * y.double().norm()).item(), (lhs, rhs)
     B = dev(mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D)))
     ys = torch.randn(gm.proj_shape(D), device="cuda")
     Axs = torch.empty_like(ys)
     mm.mm_forward(gm, B, x, K, Axs)
     mm.mm_adjoint(gm, B, ys, K, ATy)
     lhs, rhs = (Axs.double() * ys.double()).sum().item(), (x.double() * ATy.double()).sum().item()
-    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs)), (lhs, rhs)
+    assert abs(lhs - rhs) <= 1e-5 * (Axs.double().norm() * ys.double().norm()).item(), (lhs, rhs)
 
 
 def test_zero_residual_and_zero_weight(mm):
