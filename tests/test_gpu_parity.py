@@ -332,3 +332,54 @@ def test_gd_iterations_c4_recipe(ora, mm):
         assert abs(loss.item() - Lo) <= TOL_LOSS * abs(Lo)
         x_o = (x_o.astype(np.float64) - np.float32(eta).astype(np.float64) * g_o).astype(np.float32)
     assert einf(x_g.cpu().numpy()[..., :K], x_o) <= 1e-4
+
+
+def test_c5_full_size_sampled(ora, mm):
+    """BASELINE.json config 5 at FULL size (256^3, K=45, 360 projections, 256^2 detector, D=8), in the launch
+    configuration bench.py times (ldk = 48, unit weights).  The oracle cannot run the whole problem in test time, so
+    parity is checked on sampled outputs it computes one by one: rays of the model sinogram / weighted residual
+    (forward_rays) and voxels of the gradient (gradient_voxels, from scratch through the voxel's column of A).
+    Errors are scaled by the maximum of the whole GPU array (the oracle's maximum is not available at this size;
+    the two agree to the tolerance being tested).  Data is synth.surrogate_model: made by neither implementation."""
+    import torch
+    cfg = synth.get_config("C5")
+    rot, tilt = synth.angles(cfg)
+    K, D, ldk = cfg.K, cfg.D, synth.ldk_for(cfg.K)
+    vol = synth.make_volume(cfg, ldk)
+    gm = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
+    go = ora.Geometry(cfg.shape, cfg.det, rot, tilt)
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    data = synth.surrogate_model(cfg, level=float(np.abs(vol[..., 0]).max()) * 100.0)
+    dB, dvol, ddata = dev(B), dev(vol), dev(data)
+    model = torch.empty(gm.proj_shape(D), device="cuda")
+    mm.mm_forward(gm, dB, dvol, K, model)
+    grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    mm.mm_loss_gradient(gm, dB, dvol, K, ddata, None, grad, loss, wr)
+    torch.cuda.synchronize()
+    r = np.random.default_rng(55)
+    # --- sampled rays: every tilt, rays through the sample and near the detector edge
+    sjk = np.stack([r.integers(0, cfg.P, 240), r.integers(0, cfg.det[0], 240), r.integers(0, cfg.det[1], 240)], axis=1)
+    sjk[:40, 1] = r.integers(96, 160, 40); sjk[:40, 2] = r.integers(96, 160, 40)       # central rays for sure
+    want = ora.forward_rays(go, B, vol, sjk)
+    idx = tuple(torch.from_numpy(sjk[:, i].astype(np.int64)).cuda() for i in range(3))
+    got = model[idx].cpu().numpy()
+    scale = float(model.abs().max())
+    assert np.abs(want).max() > 0.05 * scale                       # the sample is not all background
+    assert np.abs(got - want).max() / scale <= TOL
+    got_wr = wr[idx].cpu().numpy()
+    assert np.abs(got_wr - (want - data[sjk[:, 0], sjk[:, 1], sjk[:, 2]])).max() / scale <= TOL
+    # --- loss: fp64 reduction of the GPU's own residuals (the residuals themselves are checked above)
+    L64 = 0.5 * float((wr.double() ** 2).sum())
+    assert abs(loss.item() - L64) <= TOL_LOSS * L64
+    # --- sampled voxels of the gradient: interior, faces, corners
+    xyz = np.concatenate([r.integers(64, 192, (10, 3)), r.integers(0, 256, (6, 3)),
+                          np.array([[0, 0, 0], [255, 255, 255], [0, 128, 255], [128, 0, 17]])]).astype(np.int32)
+    want_g = ora.gradient_voxels(go, B, vol, data, None, xyz)
+    gi = tuple(torch.from_numpy(xyz[:, i].astype(np.int64)).cuda() for i in range(3))
+    got_g = grad[gi].cpu().numpy()
+    gscale = float(grad[..., :K].abs().max())
+    assert np.abs(got_g[:, :K] - want_g).max() / gscale <= TOL
+    assert np.all(got_g[:, K:] == 0.0)
+    assert not torch.isnan(grad).any().item()
