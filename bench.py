@@ -157,6 +157,22 @@ def reference_arm(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """device-timed duration of the slowest rank (the contract's max-over-ranks); identity at world 1."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(cfg, world: int, ms_step: float) -> float:
+    """whole-job G vcp/s of `world` independent replicas ("replicas only") that each took ms_step."""
+    return world * cfg.vcp / (ms_step * 1e-3) / 1e9
+
+
 def workload_name(cfg):
     return (f"{cfg.name}: {cfg.shape[0]}x{cfg.shape[1]}x{cfg.shape[2]} voxels, l_max={cfg.ell_max} (K={cfg.K}), "
             f"P={cfg.P}, detector {cfg.det[0]}x{cfg.det[1]}, D={cfg.D}")
@@ -235,15 +251,11 @@ def ours(args, cfg):
         dist.barrier()
     launches = mm.mm_launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = start.elapsed_time(end)
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = t.item()
+    total_ms = max_over_ranks(start.elapsed_time(end), world, torch.device("cuda", local))
     ms_step = total_ms / args.steps
     fwd_ms = sum(a.elapsed_time(b) for a, b in zip(ev0, evm)) / args.steps
     adj_ms = sum(a.elapsed_time(b) for a, b in zip(evm, ev1)) / args.steps
-    value = world * cfg.vcp / (ms_step * 1e-3) / 1e9
+    value = aggregate_throughput(cfg, world, ms_step)
     loss_val = loss.item()
 
     # ---- end to end through the host-buffer C-ABI call (H2D of every input, D2H of gradient + loss, inside)

@@ -7,8 +7,9 @@
 // (2.17 T FMA on BASELINE config 5, the adjoint's dominant term): each CTA streams its
 // 128 x 16 slices of t through shared memory into tcgen05.mma (kind::tf32, M=128, N=ldk, K=8) with the fp32
 // accumulators in tensor memory.  Plain TF32 (10-bit mantissa) cannot meet the 1e-5 parity bar, so both operands
-// are split x = hi + lo with hi = x truncated to TF32 and lo = x - hi (exact), and three products are issued:
-// hi*hi + lo*hi + hi*lo (error ~2^-21 per term).
+// are split x = hi + lo with hi = x rounded to TF32 and lo = x - hi (exact), and three products are issued:
+// lo*hi + hi*lo + hi*hi (error ~2^-21 per term).  The MMA's fp32 accumulation truncates, so it is cut into
+// windows that are summed in round-to-nearest fp32 (see drain_window).
 //
 // Shared-memory operand layout (K-major, no swizzle; canonical "interleave" form): a core matrix is 8 rows x 16
 // bytes (4 tf32) stored contiguously; element (r, k) of a tile with R rows sits at
@@ -282,7 +283,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
     constexpr int NPC = KC / D;                   // projections per stage
     constexpr int A_FLOATS = TC_M * KC, B_FLOATS = NPAD * KC;
     constexpr int TCOLS = TcCols<NPAD>::value, ACCW = TcCols<NPAD>::accw;
-    constexpr int WIN = 8;                        // chunks per accumulation window (see flush_window)
+    constexpr int WIN = 8;                        // chunks per accumulation window (see drain_window)
     constexpr uint32_t IDESC = idesc_tf32(TC_M, NPAD);
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     float *sA = reinterpret_cast<float *>(smem_raw);                  // [stage][hi,lo][A_FLOATS]
