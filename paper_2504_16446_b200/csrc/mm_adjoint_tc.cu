@@ -312,25 +312,44 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
 
     if (warp == 4) {
         // ---------------- B operand + MMA issue ----------------
-        for (int ch = 0; ch < nch; ch++) {
-            const int st = ch & 1, s0 = ch * NPC;
-            if (ch >= 2) mbar_wait(&empty[st], (uint32_t)(((ch >> 1) - 1) & 1));
-            float *Bhi = sB + (2 * st) * B_FLOATS, *Blo = Bhi + B_FLOATS;
-            // element (n = channel i, k = (p, c)) = w_s B[s0+p][i][c], split hi/lo
-            for (int g = lane; g < NPAD * (KC / 4); g += 32) {
+        // element (n = channel i, k = (p, c)) of a stage's B tile = w_s B[s0+p][i][c]; its NPAD*KC/4 16-byte
+        // groups are spread over the 32 lanes.  The global loads for chunk ch+1 are issued before this warp
+        // waits for chunk ch's rows, so their latency is off the MMA's critical path.
+        constexpr int BG = (NPAD * (KC / 4) + 31) / 32;       // groups per lane
+        float4 breg[BG];
+        auto load_b = [&](int s0) {
+#pragma unroll
+            for (int i = 0; i < BG; i++) {
+                const int g = lane + 32 * i;
                 const int n = g % NPAD, kg = g / NPAD;                // 16-byte group: columns 4kg .. 4kg+3
                 const int p = (4 * kg) / D, c = (4 * kg) % D, s = s0 + p;
                 float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (n < a.K && s < a.P) {
+                if (g < NPAD * (KC / 4) && n < a.K && s < a.P) {
                     b = __ldg(reinterpret_cast<const float4 *>(a.B + ((long long)s * a.K + n) * D + c));
                     const float w = __ldg(&a.tab[s].w);
                     b.x *= w; b.y *= w; b.z *= w; b.w *= w;
                 }
-                float4 h, l;
-                split_tf32(b.x, h.x, l.x); split_tf32(b.y, h.y, l.y); split_tf32(b.z, h.z, l.z); split_tf32(b.w, h.w, l.w);
-                *reinterpret_cast<float4 *>(Bhi + kg * (NPAD * 4) + n * 4) = h;
-                *reinterpret_cast<float4 *>(Blo + kg * (NPAD * 4) + n * 4) = l;
+                breg[i] = b;
             }
+        };
+        load_b(0);
+        for (int ch = 0; ch < nch; ch++) {
+            const int st = ch & 1;
+            if (ch >= 2) mbar_wait(&empty[st], (uint32_t)(((ch >> 1) - 1) & 1));
+            float *Bhi = sB + (2 * st) * B_FLOATS, *Blo = Bhi + B_FLOATS;
+#pragma unroll
+            for (int i = 0; i < BG; i++) {
+                const int g = lane + 32 * i;
+                if (g < NPAD * (KC / 4)) {
+                    const int n = g % NPAD, kg = g / NPAD;
+                    const float4 b = breg[i];
+                    float4 h, l;
+                    split_tf32(b.x, h.x, l.x); split_tf32(b.y, h.y, l.y); split_tf32(b.z, h.z, l.z); split_tf32(b.w, h.w, l.w);
+                    *reinterpret_cast<float4 *>(Bhi + kg * (NPAD * 4) + n * 4) = h;
+                    *reinterpret_cast<float4 *>(Blo + kg * (NPAD * 4) + n * 4) = l;
+                }
+            }
+            if (ch + 1 < nch) load_b((ch + 1) * NPC);
             fence_async_smem();
             __syncwarp();
             if (lane == 0) {

@@ -30,6 +30,9 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
     return MM_OK;
 }
 
+#ifndef FWD_GS
+#define FWD_GS 8                          // projections interleaved in block order (L2 reuse across projections)
+#endif
 #ifndef FWD_MINB
 #define FWD_MINB 4
 #endif
@@ -125,10 +128,17 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
     const int q = tid % G;                        // lane within the ray's group
     const int r = tid / G;                        // ray within the block
     const int tiles_k = (a.Kd + TK - 1) / TK, tiles_j = (a.J + TJ - 1) / TJ;
-    int tile = blockIdx.x;
+    // Block order: FWD_GS consecutive projections (neighbouring rotation angles) are interleaved tile by tile, so
+    // blocks resident at the same time walk the same band of the volume for several projections and the second
+    // to FWD_GS-th reader of a voxel finds it in L2 instead of HBM.
+    const int tpp = tiles_k * tiles_j;                                   // tiles per projection
+    const int grp = blockIdx.x / (FWD_GS * tpp);
+    const int rem = blockIdx.x - grp * (FWD_GS * tpp);
+    const int gs = min(FWD_GS, a.P - grp * FWD_GS);                      // the last group may be short
+    int tile = rem / gs;
+    const int s = grp * FWD_GS + rem % gs;
     const int tk = tile % tiles_k; tile /= tiles_k;
-    const int tj = tile % tiles_j;
-    const int s = tile / tiles_j;
+    const int tj = tile;
     const int j = tj * TJ + r / TK, k = tk * TK + r % TK;
     const bool ray_ok = (j < a.J) && (k < a.Kd);
 
