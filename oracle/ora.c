@@ -327,3 +327,44 @@ void ora_dense_matrix(const ora_geom *g, int s, double *mat)
                     }
         }
 }
+
+/* NEXT-1 (reading S9, second half): the adjoint AS THE PAPER DESCRIBES IT, PAPER.md:314 — "bilinear
+ * interpolation ... of the projection for the adjoint".  Voxel-driven and NOT the transpose of joseph_ray: for each
+ * voxel x and projection s the detector position (j0,k0) of the voxel follows from Eq. 4,
+ *     j0 = jc + dj_s + (a/b) js.(x - xc),   k0 = kc + dk_s + (a/b) ks.(x - xc),
+ * the projection is interpolated bilinearly at (j0,k0) (pixels outside the detector count as 0) and the value
+ * is weighted by the same Joseph step w_s = a/|d_m| the forward uses, so both operators carry path-length units:
+ *     out[x][i] = sum_s w_s sum_{a,b in {0,1}} (a ? fj : 1-fj)(b ? fk : 1-fk) y[s][jb+a][kb+b][i].
+ * y[P][J][Kd][K] -> out[X][Y][Z][K].  Pins: tests/test_oracle_backproject.py. */
+void ora_john_backproject_bilinear(const ora_geom *g, const double *y, int K, double *out, int nthreads)
+{
+    long nvox = (long)g->shape[0] * g->shape[1] * g->shape[2];
+    double ab = g->a / g->b;
+#pragma omp parallel for schedule(dynamic, 256) num_threads(nthreads)
+    for (long q = 0; q < nvox; q++) {
+        int x[3];
+        x[2] = (int)(q % g->shape[2]); x[1] = (int)((q / g->shape[2]) % g->shape[1]);
+        x[0] = (int)(q / ((long)g->shape[2] * g->shape[1]));
+        double *acc = out + (size_t)q * K;
+        for (int i = 0; i < K; i++) acc[i] = 0.0;
+        for (int s = 0; s < g->P; s++) {
+            const double *js = g->js + 3 * s, *ks = g->ks + 3 * s;
+            double j0 = 0.5 * (g->J - 1) + g->joff[s], k0 = 0.5 * (g->Kd - 1) + g->koff[s];
+            for (int i = 0; i < 3; i++) {
+                double rel = (double)x[i] - 0.5 * (g->shape[i] - 1);
+                j0 += ab * js[i] * rel; k0 += ab * ks[i] * rel;
+            }
+            double flj = floor(j0), flk = floor(k0);
+            int jb = (int)flj, kb = (int)flk;
+            double fj = j0 - flj, fk = k0 - flk;
+            for (int da = 0; da < 2; da++)
+                for (int db = 0; db < 2; db++) {
+                    int jj = jb + da, kk = kb + db;
+                    if (jj < 0 || jj >= g->J || kk < 0 || kk >= g->Kd) continue;      /* no such pixel */
+                    double wgt = g->w[s] * (da ? fj : 1.0 - fj) * (db ? fk : 1.0 - fk);
+                    const double *yy = y + (((size_t)s * g->J + jj) * g->Kd + kk) * K;
+                    for (int i = 0; i < K; i++) acc[i] += wgt * yy[i];
+                }
+        }
+    }
+}

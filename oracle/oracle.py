@@ -10,6 +10,7 @@ What is here (numpy, fp64) and what it follows:
   basis_forward/adjoint Eq. 6 reciprocal-space map and its transpose
   forward / adjoint    A = (basis map) o (John transform), Eq. 6-8, and A^T
   loss_gradient        r = Ac - I (Eq. 13), L = 1/2 sum w r^2, grad = A^T (w r)     PAPER.md:101, 324, readings S10, S11
+  john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
 
 Pins: tests/test_oracle_sh.py, tests/test_oracle_john.py, tests/test_oracle_model.py (all CPU).
@@ -61,6 +62,7 @@ def _load():
         L.ora_voxel_taps.restype = ctypes.c_long
         L.ora_voxel_taps.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_long]
         L.ora_dense_matrix.argtypes = [ctypes.c_void_p, ctypes.c_int, dp]
+        L.ora_john_backproject_bilinear.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp, ctypes.c_int]
         _lib = L
     return _lib
 
@@ -163,6 +165,22 @@ def john_adjoint(g: Geometry, y, form="gather", threads=None):
     else:
         _load().ora_john_adjoint_gather(g._h, _dp(y), K, _dp(out), threads or default_threads())
     return out
+
+
+def john_backproject_bilinear(g: Geometry, y, threads=None):
+    """out[X][Y][Z][K] float64: the paper's own (unmatched) adjoint, PAPER.md:314 — voxel-driven bilinear
+    interpolation of the projection y[P][J][Kd][K] at the voxel's detector position, weighted by w_s (NEXT-1)."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    K = y.shape[-1]
+    assert y.shape == (g.P,) + g.det + (K,)
+    out = np.empty(g.shape + (K,), dtype=np.float64)
+    _load().ora_john_backproject_bilinear(g._h, _dp(y), K, _dp(out), threads or default_threads())
+    return out
+
+
+def backproject_bilinear(g: Geometry, B, sino, threads=None):
+    """basis^T (Eq. 6 transposed) followed by the paper's bilinear back-projection."""
+    return john_backproject_bilinear(g, basis_adjoint(B, sino), threads=threads)
 
 
 def john_adjoint_voxels(g: Geometry, y, xyz, threads=None):
