@@ -258,6 +258,20 @@ def ours(args, cfg):
     value = aggregate_throughput(cfg, world, ms_step)
     loss_val = loss.item()
 
+    # ---- optional extra (not part of the step): the paper's bilinear back-projection (NEXT-1) of the residual
+    extras = None
+    if args.extras and rank == 0:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        mm.mm_backproject(g, B, wr, K, grad)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            mm.mm_backproject(g, B, wr, K, grad)
+        e1.record()
+        torch.cuda.synchronize()
+        extras = {"mm_backproject_ms": e0.elapsed_time(e1) / args.steps,
+                  "what": "basis^T + bilinear interpolation of the projection (PAPER.md:314), same wr as the step"}
+
     # ---- end to end through the host-buffer C-ABI call (H2D of every input, D2H of gradient + loss, inside)
     e2e = None
     if rank == 0:
@@ -311,7 +325,7 @@ def ours(args, cfg):
             "config": {"workload": workload_name(cfg), "ldk": ldk, "l2": "inputs (%.1f GB volume) larger than L2; no flush" % (vol.numel() * 4 / 1e9),
                        "multi_gpu": "replicas only", "input_generation_s": round(gen_s, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "loss": loss_val, "phase_ms": {"forward_residual": fwd_ms, "adjoint": adj_ms}}
+            "loss": loss_val, "phase_ms": {"forward_residual": fwd_ms, "adjoint": adj_ms}, "extras": extras}
     print(json.dumps(line), flush=True)
 
 
@@ -323,6 +337,7 @@ def main():
     ap.add_argument("--config", default="C5", choices=sorted(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true", help="also time mm_backproject (outside the step)")
     args = ap.parse_args()
     cfg = synth.get_config(args.config)
     if args.impl == "reference":

@@ -125,6 +125,18 @@ mm_status mm_forward(const mm_geometry *g, const float *B, const float *vol, int
 mm_status mm_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,
                      float *vol_out, void *stream);
 
+/* NEXT-1 — the adjoint as the paper words it (Joseph's method "using bilinear interpolation of the field
+ * for the forward and the projection for the adjoint"): voxel-driven, NOT the transpose of mm_john_forward
+ * (reading S9).  For every voxel x and projection s, with (j0,k0) the detector position of x (Eq. 4),
+ *   vol_out[x][i] = sum_s w_s * bilinear(proj[s])(j0, k0)_i,   pixels outside the detector count as 0.
+ * mm_john_backproject: proj [P][J][Kd][ldk] DEVICE in -> vol_out [X][Y][Z][ldk] DEVICE out (overwritten).
+ * mm_backproject: the same applied to basis^T sino, fused (sino [P][J][Kd][D] DEVICE in); this is the pair
+ * (forward, back-projection) the paper's SIRT/MITRA iterations use. */
+mm_status mm_john_backproject(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out,
+                              void *stream);
+mm_status mm_backproject(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,
+                         float *vol_out, void *stream);
+
 /* One fused gradient evaluation (Eq. 9 data term with a = 2, Eq. 13; S10, S11):
  *   phase 1 (all rays):   r = (A vol) - data;  wr = weights * r;  *loss = 1/2 sum weights r^2
  *   phase 2 (all voxels): grad = A^T wr

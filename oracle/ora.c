@@ -336,35 +336,49 @@ void ora_dense_matrix(const ora_geom *g, int s, double *mat)
  * is weighted by the same Joseph step w_s = a/|d_m| the forward uses, so both operators carry path-length units:
  *     out[x][i] = sum_s w_s sum_{a,b in {0,1}} (a ? fj : 1-fj)(b ? fk : 1-fk) y[s][jb+a][kb+b][i].
  * y[P][J][Kd][K] -> out[X][Y][Z][K].  Pins: tests/test_oracle_backproject.py. */
+static void backproject_voxel(const ora_geom *g, const double *y, int K, const int x[3], double *acc)
+{
+    double ab = g->a / g->b;
+    for (int i = 0; i < K; i++) acc[i] = 0.0;
+    for (int s = 0; s < g->P; s++) {
+        const double *js = g->js + 3 * s, *ks = g->ks + 3 * s;
+        double j0 = 0.5 * (g->J - 1) + g->joff[s], k0 = 0.5 * (g->Kd - 1) + g->koff[s];
+        for (int i = 0; i < 3; i++) {
+            double rel = (double)x[i] - 0.5 * (g->shape[i] - 1);
+            j0 += ab * js[i] * rel; k0 += ab * ks[i] * rel;
+        }
+        double flj = floor(j0), flk = floor(k0);
+        int jb = (int)flj, kb = (int)flk;
+        double fj = j0 - flj, fk = k0 - flk;
+        for (int da = 0; da < 2; da++)
+            for (int db = 0; db < 2; db++) {
+                int jj = jb + da, kk = kb + db;
+                if (jj < 0 || jj >= g->J || kk < 0 || kk >= g->Kd) continue;      /* no such pixel */
+                double wgt = g->w[s] * (da ? fj : 1.0 - fj) * (db ? fk : 1.0 - fk);
+                const double *yy = y + (((size_t)s * g->J + jj) * g->Kd + kk) * K;
+                for (int i = 0; i < K; i++) acc[i] += wgt * yy[i];
+            }
+    }
+}
+
 void ora_john_backproject_bilinear(const ora_geom *g, const double *y, int K, double *out, int nthreads)
 {
     long nvox = (long)g->shape[0] * g->shape[1] * g->shape[2];
-    double ab = g->a / g->b;
 #pragma omp parallel for schedule(dynamic, 256) num_threads(nthreads)
     for (long q = 0; q < nvox; q++) {
         int x[3];
         x[2] = (int)(q % g->shape[2]); x[1] = (int)((q / g->shape[2]) % g->shape[1]);
         x[0] = (int)(q / ((long)g->shape[2] * g->shape[1]));
-        double *acc = out + (size_t)q * K;
-        for (int i = 0; i < K; i++) acc[i] = 0.0;
-        for (int s = 0; s < g->P; s++) {
-            const double *js = g->js + 3 * s, *ks = g->ks + 3 * s;
-            double j0 = 0.5 * (g->J - 1) + g->joff[s], k0 = 0.5 * (g->Kd - 1) + g->koff[s];
-            for (int i = 0; i < 3; i++) {
-                double rel = (double)x[i] - 0.5 * (g->shape[i] - 1);
-                j0 += ab * js[i] * rel; k0 += ab * ks[i] * rel;
-            }
-            double flj = floor(j0), flk = floor(k0);
-            int jb = (int)flj, kb = (int)flk;
-            double fj = j0 - flj, fk = k0 - flk;
-            for (int da = 0; da < 2; da++)
-                for (int db = 0; db < 2; db++) {
-                    int jj = jb + da, kk = kb + db;
-                    if (jj < 0 || jj >= g->J || kk < 0 || kk >= g->Kd) continue;      /* no such pixel */
-                    double wgt = g->w[s] * (da ? fj : 1.0 - fj) * (db ? fk : 1.0 - fk);
-                    const double *yy = y + (((size_t)s * g->J + jj) * g->Kd + kk) * K;
-                    for (int i = 0; i < K; i++) acc[i] += wgt * yy[i];
-                }
-        }
+        backproject_voxel(g, y, K, x, out + (size_t)q * K);
+    }
+}
+
+/* sampled voxels xyz[nvox][3] -> out[nvox][K] (full-size parity samples) */
+void ora_john_backproject_bilinear_voxels(const ora_geom *g, const double *y, int K, long nvox, const int32_t *xyz,
+                                          double *out)
+{
+    for (long q = 0; q < nvox; q++) {
+        int x[3] = {xyz[3 * q], xyz[3 * q + 1], xyz[3 * q + 2]};
+        backproject_voxel(g, y, K, x, out + (size_t)q * K);
     }
 }

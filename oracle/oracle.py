@@ -63,6 +63,7 @@ def _load():
         L.ora_voxel_taps.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_long]
         L.ora_dense_matrix.argtypes = [ctypes.c_void_p, ctypes.c_int, dp]
         L.ora_john_backproject_bilinear.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp, ctypes.c_int]
+        L.ora_john_backproject_bilinear_voxels.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, ctypes.c_long, ip, dp]
         _lib = L
     return _lib
 
@@ -175,6 +176,16 @@ def john_backproject_bilinear(g: Geometry, y, threads=None):
     assert y.shape == (g.P,) + g.det + (K,)
     out = np.empty(g.shape + (K,), dtype=np.float64)
     _load().ora_john_backproject_bilinear(g._h, _dp(y), K, _dp(out), threads or default_threads())
+    return out
+
+
+def john_backproject_bilinear_voxels(g: Geometry, y, xyz):
+    """john_backproject_bilinear at sampled voxels xyz[n][3] -> [n][K]."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    K = y.shape[-1]
+    xyz = np.ascontiguousarray(xyz, dtype=np.int32).reshape(-1, 3)
+    out = np.empty((xyz.shape[0], K), dtype=np.float64)
+    _load().ora_john_backproject_bilinear_voxels(g._h, _dp(y), K, xyz.shape[0], _ip(xyz), _dp(out))
     return out
 
 

@@ -387,13 +387,14 @@ __global__ void __launch_bounds__(256) john_adjoint_kernel(const AdjArgs a)
         const float fj = (float)(j0 - fj0), fk = (float)(k0 - fk0);
         const float hj = pg->hj, hk = pg->hk, w = pg->w;
         const float mju = pg->mju, mku = pg->mku, mjv = pg->mjv, mkv = pg->mkv;
-        const int djlo = max((int)ceilf(fj - hj), -jb), djhi = min((int)floorf(fj + hj), a.J - 1 - jb);
-        const int dklo = max((int)ceilf(fk - hk), -kb), dkhi = min((int)floorf(fk + hk), a.Kd - 1 - kb);
+        // bilinear mode: the four pixels around (j0,k0) with weights (1-fj | fj)(1-fk | fk)
+        const int djlo = max(a.bilinear ? 0 : (int)ceilf(fj - hj), -jb), djhi = min(a.bilinear ? 1 : (int)floorf(fj + hj), a.J - 1 - jb);
+        const int dklo = max(a.bilinear ? 0 : (int)ceilf(fk - hk), -kb), dkhi = min(a.bilinear ? 1 : (int)floorf(fk + hk), a.Kd - 1 - kb);
         for (int dj = djlo; dj <= djhi; dj++) {
             const float ej = (float)dj - fj;
             for (int dk = dklo; dk <= dkhi; dk++) {
                 const float ek = (float)dk - fk;
-                const float du = fmaf(mju, ej, mku * ek), dv = fmaf(mjv, ej, mkv * ek);
+                const float du = a.bilinear ? ej : fmaf(mju, ej, mku * ek), dv = a.bilinear ? ek : fmaf(mjv, ej, mkv * ek);
                 const float wt = w * fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
                 if (wt > 0.f) {
                     const float *p = a.src + (((long long)s * a.J + (jb + dj)) * a.Kd + (kb + dk)) * a.ldk;
@@ -479,13 +480,13 @@ __global__ void __launch_bounds__(128) adjoint_fused_kernel(const AdjArgs a)
             const double fj0 = floor(j0), fk0 = floor(k0);
             const int jb = (int)fj0, kb = (int)fk0;
             const float fj = (float)(j0 - fj0), fk = (float)(k0 - fk0);
-            const int djlo = max((int)ceilf(fj - pg.hj), -jb), djhi = min((int)floorf(fj + pg.hj), a.J - 1 - jb);
-            const int dklo = max((int)ceilf(fk - pg.hk), -kb), dkhi = min((int)floorf(fk + pg.hk), a.Kd - 1 - kb);
+            const int djlo = max(a.bilinear ? 0 : (int)ceilf(fj - pg.hj), -jb), djhi = min(a.bilinear ? 1 : (int)floorf(fj + pg.hj), a.J - 1 - jb);
+            const int dklo = max(a.bilinear ? 0 : (int)ceilf(fk - pg.hk), -kb), dkhi = min(a.bilinear ? 1 : (int)floorf(fk + pg.hk), a.Kd - 1 - kb);
             for (int dj = djlo; dj <= djhi; dj++) {
                 const float ej = (float)dj - fj;
                 for (int dk = dklo; dk <= dkhi; dk++) {
                     const float ek = (float)dk - fk;
-                    const float du = fmaf(pg.mju, ej, pg.mku * ek), dv = fmaf(pg.mjv, ej, pg.mkv * ek);
+                    const float du = a.bilinear ? ej : fmaf(pg.mju, ej, pg.mku * ek), dv = a.bilinear ? ek : fmaf(pg.mjv, ej, pg.mkv * ek);
                     const float wt = pg.w * fmaxf(0.f, 1.f - fabsf(du)) * fmaxf(0.f, 1.f - fabsf(dv));
                     if (wt > 0.f) {
                         const float *p = a.src + (((long long)s * a.J + (jb + dj)) * a.Kd + (kb + dk)) * a.D;
@@ -652,7 +653,7 @@ void fill_adj(AdjArgs &a, const mm_geometry *g, const float *src, const float *B
 {
     a.tab = g->d_table; a.src = src; a.B = B; a.out = out; a.K = K; a.ldk = ldk; a.D = D;
     a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
-    a.vec_ok = 0;
+    a.vec_ok = 0; a.bilinear = 0;
 }
 
 template <int VEC, int G, int NQ>
@@ -677,10 +678,11 @@ mm_status launch_adj_fused(const AdjArgs &a, cudaStream_t st)
 }
 
 mm_status run_adjoint_fused(const mm_geometry *g, const float *B, const float *sino, int K, int ldk, int D,
-                            float *out, cudaStream_t st)
+                            float *out, cudaStream_t st, int bilinear = 0)
 {
     AdjArgs a;
     fill_adj(a, g, sino, B, out, K, ldk, D);
+    a.bilinear = bilinear;
     a.vec_ok = (D % 4 == 0) && aligned16(sino);
     static const bool tc_off = getenv("MM_DISABLE_TC") != nullptr;     // debugging switch: CUDA-core contraction
     if (!tc_off && mm_adjoint_tc_supported(a)) {
@@ -727,13 +729,15 @@ extern "C" mm_status mm_forward(const mm_geometry *g, const float *B, const floa
     return dispatch_fwd_d<1>(a, vec, (cudaStream_t)stream);
 }
 
-extern "C" mm_status mm_john_adjoint(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out, void *stream)
+static mm_status run_john_adjoint(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out, void *stream,
+                                  int bilinear, const char *who)
 {
-    mm_status st = check_common(g, K, ldk, "mm_john_adjoint");
+    mm_status st = check_common(g, K, ldk, who);
     if (st != MM_OK) return st;
-    if (!proj || !vol_out) { mm_set_error("mm_john_adjoint: NULL buffer"); return MM_ERR_NULL; }
+    if (!proj || !vol_out) { mm_set_error(std::string(who) + ": NULL buffer"); return MM_ERR_NULL; }
     AdjArgs a;
     fill_adj(a, g, proj, nullptr, vol_out, K, ldk, 0);
+    a.bilinear = bilinear;
     cudaStream_t cs = (cudaStream_t)stream;
     if ((ldk % 4 == 0) && aligned16(proj) && aligned16(vol_out)) {
         const int lpv = ldk / 4;
@@ -749,6 +753,26 @@ extern "C" mm_status mm_john_adjoint(const mm_geometry *g, const float *proj, in
         else launch_adj<1, 32, 8>(a, cs);
     }
     return check_launch("john_adjoint_kernel");
+}
+
+extern "C" mm_status mm_john_adjoint(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out, void *stream)
+{
+    return run_john_adjoint(g, proj, K, ldk, vol_out, stream, 0, "mm_john_adjoint");
+}
+
+extern "C" mm_status mm_john_backproject(const mm_geometry *g, const float *proj, int32_t K, int32_t ldk, float *vol_out, void *stream)
+{
+    return run_john_adjoint(g, proj, K, ldk, vol_out, stream, 1, "mm_john_backproject");
+}
+
+extern "C" mm_status mm_backproject(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,
+                                    float *vol_out, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_backproject");
+    if (st != MM_OK) return st;
+    if (!B || !sino || !vol_out) { mm_set_error("mm_backproject: NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_backproject: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    return run_adjoint_fused(g, B, sino, K, ldk, D, vol_out, (cudaStream_t)stream, 1);
 }
 
 extern "C" mm_status mm_adjoint(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk, int32_t D,

@@ -18,7 +18,7 @@ _lib = None
 
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
-           "mm_adjoint", "mm_loss_gradient", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
+           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -56,6 +56,8 @@ def load():
     L.mm_basis_adjoint.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_forward.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_adjoint.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mm_john_backproject.argtypes = [vp, vp, i32, i32, vp, vp]
+    L.mm_backproject.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_loss_gradient.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     L.mm_axpy.argtypes = [vp, vp, ctypes.c_float, i64, vp]
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
@@ -201,6 +203,20 @@ def mm_adjoint(g: Geometry, B, sino, K: int, vol_out, stream=None):
     ldk, D = vol_out.shape[-1], B.shape[-1]
     _check(load().mm_adjoint(g._h, _dev(B, (g.P, K, D), "B"), _dev(sino, g.proj_shape(D), "sino"), K, ldk, D,
                              _dev(vol_out, g.vol_shape(ldk), "vol_out"), _stream(stream)), "mm_adjoint")
+    return vol_out
+
+
+def mm_john_backproject(g: Geometry, proj, K: int, vol_out, stream=None):
+    ldk = proj.shape[-1]
+    _check(load().mm_john_backproject(g._h, _dev(proj, g.proj_shape(ldk), "proj"), K, ldk,
+                                      _dev(vol_out, g.vol_shape(ldk), "vol_out"), _stream(stream)), "mm_john_backproject")
+    return vol_out
+
+
+def mm_backproject(g: Geometry, B, sino, K: int, vol_out, stream=None):
+    ldk, D = vol_out.shape[-1], B.shape[-1]
+    _check(load().mm_backproject(g._h, _dev(B, (g.P, K, D), "B"), _dev(sino, g.proj_shape(D), "sino"), K, ldk, D,
+                                 _dev(vol_out, g.vol_shape(ldk), "vol_out"), _stream(stream)), "mm_backproject")
     return vol_out
 
 

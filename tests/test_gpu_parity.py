@@ -126,6 +126,17 @@ def run_all_ops(ora, mm, c, check_fused_composition=True, sh_basis=None):
     got = vout2.cpu().numpy()
     errs["adjoint"] = einf(got[..., :K], want)
     assert np.all(got[..., K:] == 0.0)
+    # --- NEXT-1: the paper's bilinear back-projection, K-channel and fused with basis^T
+    vb = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    mm.mm_john_backproject(gm, dy, K, vb)
+    got = vb.cpu().numpy()
+    errs["john_backproject"] = einf(got[..., :K], ora.john_backproject_bilinear(go, c.y[..., :K]))
+    assert np.all(got[..., K:] == 0.0)
+    vb.fill_(float("nan"))
+    mm.mm_backproject(gm, dB, dsino, K, vb)
+    got = vb.cpu().numpy()
+    errs["backproject"] = einf(got[..., :K], ora.backproject_bilinear(go, B, c.sino))
+    assert np.all(got[..., K:] == 0.0)
     # --- fused gradient (a8)
     scale = float(np.abs(want_model).max())
     data = (want_model + 0.1 * scale * c.data).astype(np.float32)          # data near the model: no giant residuals
@@ -383,3 +394,14 @@ def test_c5_full_size_sampled(ora, mm):
     assert np.abs(got_g[:, :K] - want_g).max() / gscale <= TOL
     assert np.all(got_g[:, K:] == 0.0)
     assert not torch.isnan(grad).any().item()
+    # --- NEXT-1 at full size: the paper's bilinear back-projection of the weighted residual, same sampled voxels
+    mm.mm_backproject(gm, dB, wr, K, grad)
+    # (projection by projection: back-project the D channels, then apply that projection's B^T — the K-channel
+    # sinogram of the whole problem would not fit the oracle's budget)
+    wr_h = wr.cpu().numpy()
+    want_b = np.zeros((xyz.shape[0], K))
+    for s in range(cfg.P):
+        g1 = ora.Geometry(cfg.shape, cfg.det, rot[s:s + 1], tilt[s:s + 1])
+        want_b += ora.john_backproject_bilinear_voxels(g1, wr_h[s:s + 1].astype(np.float64), xyz) @ B[s].astype(np.float64).T
+    got_b = grad[gi].cpu().numpy()
+    assert np.abs(got_b[:, :K] - want_b).max() / float(grad[..., :K].abs().max()) <= TOL

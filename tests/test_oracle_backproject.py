@@ -99,3 +99,12 @@ def test_channels_independent_and_outside_is_zero(ora):
     full = ora.john_backproject_bilinear(g2, y)
     for i in range(3):
         assert np.array_equal(full[..., i], ora.john_backproject_bilinear(g2, y[..., i:i + 1])[..., 0])
+
+
+def test_sampled_voxels_equal_full(ora):
+    shape, det = (6, 5, 7), (8, 9)
+    g = ora.Geometry(shape, det, [0.4, 1.9, 3.0], [0.2, -0.3, 0.6])
+    y = np.random.default_rng(9).standard_normal((3,) + det + (2,))
+    full = ora.john_backproject_bilinear(g, y)
+    xyz = np.array([[0, 0, 0], [5, 4, 6], [2, 3, 1], [3, 0, 6]])
+    assert np.array_equal(ora.john_backproject_bilinear_voxels(g, y, xyz), full[xyz[:, 0], xyz[:, 1], xyz[:, 2]])
