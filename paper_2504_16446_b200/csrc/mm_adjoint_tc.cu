@@ -260,6 +260,38 @@ __device__ __forceinline__ void gather_voxel_fixed(const TcProj &pg, const float
         for (int i = 0; i < D; i++) t[i] = fmaf(wt[n], v[n][i], t[i]);
 }
 
+// The paper's own adjoint ("bilinear interpolation of the projection"; NEXT-1): the four pixels
+// around the voxel's detector position with weights (1-fj | fj)(1-fk | fk); pixels off the detector count as 0.
+template <int D>
+__device__ __forceinline__ void gather_voxel_bilinear(const TcProj &pg, const float *__restrict__ src_s, int x, int y, int z,
+                                                      int J, int Kd, float (&t)[D])
+{
+#pragma unroll
+    for (int c = 0; c < D; c++) t[c] = 0.f;
+    const double j0 = fma((double)x, pg.Jx0, fma((double)y, pg.Jx1, fma((double)z, pg.Jx2, pg.Jc)));
+    const double k0 = fma((double)x, pg.Kx0, fma((double)y, pg.Kx1, fma((double)z, pg.Kx2, pg.Kc)));
+    const int jb = __double2int_rd(j0), kb = __double2int_rd(k0);
+    const float fj = (float)(j0 - (double)jb), fk = (float)(k0 - (double)kb);
+    const float4 *src4 = reinterpret_cast<const float4 *>(src_s);
+    const int i00 = (jb * Kd + kb) * (D / 4), rstep = Kd * (D / 4);
+    float wt[4], v[4][D];
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+            const bool on = (unsigned)(jb + r) < (unsigned)J && (unsigned)(kb + c) < (unsigned)Kd;
+            wt[2 * r + c] = (r ? fj : 1.f - fj) * (c ? fk : 1.f - fk);
+            const float4 *p = src4 + (i00 + r * rstep + c * (D / 4));
+#pragma unroll
+            for (int q = 0; q < D; q += 8) ldg256_pred(p + q / 4, on, &v[2 * r + c][q]);
+        }
+    }
+#pragma unroll
+    for (int n = 0; n < 4; n++)
+#pragma unroll
+        for (int i = 0; i < D; i++) t[i] = fmaf(wt[n], v[n][i], t[i]);
+}
+
 // two regions of ACCW columns each: the MMA accumulator of the current window, and the running sum
 template <int NPAD>
 struct TcCols {
@@ -423,6 +455,13 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
                 float t[D];
                 const TcProj &pg = wsp[p];
                 const float *src_s = a.src + (long long)min(s0 + p, a.P - 1) * proj_stride;
+                if (a.bilinear) {
+                    if (pg.valid) gather_voxel_bilinear<D>(pg, src_s, x, y, z, a.J, a.Kd, t);
+                    else {
+#pragma unroll
+                        for (int c = 0; c < D; c++) t[c] = 0.f;
+                    }
+                } else
                 switch (pg.valid) {                                   // uniform across the block
                     case 4: gather_voxel_fixed<D, 2, 2>(pg, src_s, x, y, z, a.J, a.Kd, t); break;
                     case 5: gather_voxel_fixed<D, 2, 3>(pg, src_s, x, y, z, a.J, a.Kd, t); break;

@@ -405,3 +405,14 @@ def test_c5_full_size_sampled(ora, mm):
         want_b += ora.john_backproject_bilinear_voxels(g1, wr_h[s:s + 1].astype(np.float64), xyz) @ B[s].astype(np.float64).T
     got_b = grad[gi].cpu().numpy()
     assert np.abs(got_b[:, :K] - want_b).max() / float(grad[..., :K].abs().max()) <= TOL
+
+
+@pytest.mark.parametrize("K,ldk,D,P", [(13, 16, 8, 7), (13, 16, 16, 5), (30, 32, 8, 19), (45, 48, 16, 9), (60, 64, 8, 17),
+                                        (61, 64, 16, 33)])
+def test_tensor_core_adjoint_instantiations(ora, mm, K, ldk, D, P):
+    """every (D, accumulator width) instantiation of the tcgen05 adjoint, with projection counts that leave a
+    short last chunk (P odd), fewer chunks than one accumulation window, and more than two windows."""
+    r = np.random.default_rng(100 * K + D)
+    c = Case((19, 17, 21), (24, 22), r.uniform(0, 2 * math.pi, P), r.uniform(-0.75, 0.75, P), K, ldk, D, seed=K + D,
+             joff=r.uniform(-1, 1, P), koff=r.uniform(-1, 1, P))
+    assert_errs(run_all_ops(ora, mm, c))
