@@ -11,6 +11,7 @@ What is here (numpy, fp64) and what it follows:
   forward / adjoint    A = (basis map) o (John transform), Eq. 6-8, and A^T
   loss_gradient        r = Ac - I (Eq. 13), L = 1/2 sum w r^2, grad = A^T (w r)     PAPER.md:101, 324, readings S10, S11
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
+  sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
 
 Pins: tests/test_oracle_sh.py, tests/test_oracle_john.py, tests/test_oracle_model.py (all CPU).
@@ -348,3 +349,32 @@ def gradient_voxels(g: Geometry, B, vol, data, weights, xyz, threads=None):
         wr = r if weights is None else r * np.asarray(weights[s, j, k], dtype=np.float64)
         out[q] = np.einsum("n,nic,nc->i", taps[:, 3], B[s], wr)
     return out
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1 (second half): SIRT / MITRA as preconditioned weighted least squares
+# ------------------------------------------------------------------------------------------------
+def sirt_preconditioners(g: Geometry, B, matched=False, floor=1e-6, threads=None):
+    """(W[P][J][Kd][D], C[X][Y][Z][K]) of the SIRT/MITRA iteration ("the weight-preconditioner approach
+    ... can also be extended to the RSM").  The paper gives no formula; reading S19: the classical SIRT
+    choice on the entrywise absolute value of the system matrix, |A|_s = P_s (x) |B_s| (P >= 0):
+        W = 1 / (|A| 1)   (inverse row sums),      C = 1 / (|A|' 1)   (inverse column sums),
+    with |A|' the back-projector the iteration itself uses (exact transpose if matched, else the paper's bilinear
+    one), and 0 where a sum does not exceed `floor` (rays that miss the sample, voxels no ray sees)."""
+    absB = np.abs(np.asarray(B, dtype=np.float64))
+    K, D = absB.shape[1], absB.shape[2]
+    rows = forward(g, absB, np.ones(g.shape + (K,), dtype=np.float32), threads)
+    ones = np.ones((g.P,) + g.det + (D,), dtype=np.float64)
+    cols = adjoint(g, absB, ones, form="scatter") if matched else backproject_bilinear(g, absB, ones, threads)
+    W = np.where(rows > floor, 1.0 / np.maximum(rows, floor), 0.0)
+    C = np.where(cols > floor, 1.0 / np.maximum(cols, floor), 0.0)
+    return W, C
+
+
+def sirt_step(g: Geometry, B, vol, data, W, C, matched=False, threads=None):
+    """one iteration  c <- c - C (.) A'( W (.) (A c - I) )  (ref. 45); returns (c_new, L) with
+    L = 1/2 sum W r^2 evaluated at the incoming c."""
+    r = forward(g, B, np.asarray(vol, dtype=np.float32), threads) - np.asarray(data, dtype=np.float64)
+    wr = W * r
+    back = adjoint(g, B, wr, form="scatter") if matched else backproject_bilinear(g, B, wr, threads)
+    return np.asarray(vol, dtype=np.float64) - C * back, 0.5 * float(np.sum(wr * r))
