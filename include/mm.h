@@ -146,6 +146,19 @@ mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vo
                            int32_t D, const float *data, const float *weights, float *grad, double *loss,
                            float *wr_workspace, void *stream);
 
+/* Phase 1 of mm_loss_gradient alone: wr = weights * (A vol - data), *loss = 1/2 sum weights r^2; lets a caller
+ * pair the forward with the back-projector of its choice (mm_adjoint or mm_backproject), as SIRT/MITRA do.
+ * Same arguments as mm_loss_gradient; wr [P][J][Kd][D] DEVICE out. */
+mm_status mm_residual_loss(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                           const float *data, const float *weights, float *wr, double *loss, void *stream);
+
+/* SIRT / MITRA building blocks (SIRT as preconditioned weighted least squares; reading S19).
+ * mm_reciprocal: x[i] <- 1/x[i] where x[i] > floor, else 0 — turns row sums |A| 1 (mm_forward of an all-ones
+ *   volume with |B|) into the weights W and column sums |A|' 1 into the preconditioner C; n floats, DEVICE, in place.
+ * mm_axpy_precond: c[i] <- c[i] - eta * pre[i] * grad[i] — the preconditioned update c <- c - C (.) A'(W r). */
+mm_status mm_reciprocal(float *x, int64_t n, float floor, void *stream);
+mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float eta, int64_t n, void *stream);
+
 /* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */
 mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream);
 

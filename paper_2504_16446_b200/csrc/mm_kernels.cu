@@ -570,6 +570,20 @@ __global__ void axpy_kernel(float *__restrict__ c, const float *__restrict__ g, 
     if (i < n) c[i] = fmaf(-eta, g[i], c[i]);
 }
 
+// SIRT/MITRA: x <- 1/x where x > floor, else 0 (rays that miss the sample, unseen voxels)
+__global__ void reciprocal_kernel(float *__restrict__ x, float floor_, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { const float v = x[i]; x[i] = v > floor_ ? 1.f / v : 0.f; }
+}
+
+// preconditioned update c <- c - eta * pre (.) g
+__global__ void axpy_precond_kernel(float *__restrict__ c, const float *__restrict__ g, const float *__restrict__ pre, float eta, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) c[i] = fmaf(-eta * pre[i], g[i], c[i]);
+}
+
 // ================================================================================================
 // host-side dispatch
 // ================================================================================================
@@ -809,30 +823,62 @@ extern "C" mm_status mm_basis_adjoint(const mm_geometry *g, const float *B, cons
     return check_launch("basis_adjoint_kernel");
 }
 
-extern "C" mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
-                                      const float *data, const float *weights, float *grad, double *loss,
-                                      float *wr_workspace, void *stream)
+static mm_status run_residual_loss(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                   const float *data, const float *weights, float *wr, double *loss, cudaStream_t cs,
+                                   const char *who)
 {
-    mm_status st = check_common(g, K, ldk, "mm_loss_gradient");
+    mm_status st = check_common(g, K, ldk, who);
     if (st != MM_OK) return st;
-    if (!B || !vol || !data || !grad || !loss || !wr_workspace) { mm_set_error("mm_loss_gradient: NULL buffer"); return MM_ERR_NULL; }
-    if (D < 1 || D > MM_MAX_D) { mm_set_error("mm_loss_gradient: need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
-    cudaStream_t cs = (cudaStream_t)stream;
+    if (!B || !vol || !data || !loss || !wr) { mm_set_error(std::string(who) + ": NULL buffer"); return MM_ERR_NULL; }
+    if (D < 1 || D > MM_MAX_D) { mm_set_error(std::string(who) + ": need 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
     if (cudaMemsetAsync(loss, 0, sizeof(double), cs) != cudaSuccess) {
         mm_set_error(std::string("cudaMemsetAsync(loss): ") + cudaGetErrorString(cudaGetLastError()));
         return MM_ERR_CUDA;
     }
     FwdArgs a;
     fill_fwd(a, g, vol, K, ldk);
-    a.B = B; a.D = D; a.data = data; a.weights = weights; a.sino = wr_workspace; a.loss = loss;
+    a.B = B; a.D = D; a.data = data; a.weights = weights; a.sino = wr; a.loss = loss;
     const bool vec = (ldk % 4 == 0) && aligned16(vol);
-    st = dispatch_fwd_d<2>(a, vec, cs);                       // phase 1: a3 + a4 + a5
+    return dispatch_fwd_d<2>(a, vec, cs);                     // a3 + a4 + a5
+}
+
+extern "C" mm_status mm_residual_loss(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                      const float *data, const float *weights, float *wr, double *loss, void *stream)
+{
+    return run_residual_loss(g, B, vol, K, ldk, D, data, weights, wr, loss, (cudaStream_t)stream, "mm_residual_loss");
+}
+
+extern "C" mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                      const float *data, const float *weights, float *grad, double *loss,
+                                      float *wr_workspace, void *stream)
+{
+    if (!grad) { mm_set_error("mm_loss_gradient: NULL buffer"); return MM_ERR_NULL; }
+    cudaStream_t cs = (cudaStream_t)stream;
+    mm_status st = run_residual_loss(g, B, vol, K, ldk, D, data, weights, wr_workspace, loss, cs, "mm_loss_gradient");   // phase 1
     if (st != MM_OK) return st;
     if (g_phase_event && cudaEventRecord(g_phase_event, cs) != cudaSuccess) {
         mm_set_error(std::string("cudaEventRecord(phase event): ") + cudaGetErrorString(cudaGetLastError()));
         return MM_ERR_CUDA;
     }
     return run_adjoint_fused(g, B, wr_workspace, K, ldk, D, grad, cs);   // phase 2: a6 + a7
+}
+
+extern "C" mm_status mm_reciprocal(float *x, int64_t n, float floor_, void *stream)
+{
+    if (!x) { mm_set_error("mm_reciprocal: NULL buffer"); return MM_ERR_NULL; }
+    if (n < 0) { mm_set_error("mm_reciprocal: n < 0"); return MM_ERR_SHAPE; }
+    if (n == 0) return MM_OK;
+    reciprocal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, floor_, (long long)n);
+    return check_launch("reciprocal_kernel");
+}
+
+extern "C" mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float eta, int64_t n, void *stream)
+{
+    if (!c || !grad || !pre) { mm_set_error("mm_axpy_precond: NULL buffer"); return MM_ERR_NULL; }
+    if (n < 0) { mm_set_error("mm_axpy_precond: n < 0"); return MM_ERR_SHAPE; }
+    if (n == 0) return MM_OK;
+    axpy_precond_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c, grad, pre, eta, (long long)n);
+    return check_launch("axpy_precond_kernel");
 }
 
 extern "C" mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream)

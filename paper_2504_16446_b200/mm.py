@@ -18,7 +18,8 @@ _lib = None
 
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
-           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
+           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_residual_loss", "mm_reciprocal",
+           "mm_axpy_precond", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -60,6 +61,9 @@ def load():
     L.mm_backproject.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_loss_gradient.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     L.mm_axpy.argtypes = [vp, vp, ctypes.c_float, i64, vp]
+    L.mm_residual_loss.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp]
+    L.mm_reciprocal.argtypes = [vp, i64, ctypes.c_float, vp]
+    L.mm_axpy_precond.argtypes = [vp, vp, vp, ctypes.c_float, i64, vp]
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
     L.mm_set_phase_event.argtypes = [vp]
     L.mm_launch_count.restype = i64
@@ -231,6 +235,27 @@ def mm_loss_gradient(g: Geometry, B, vol, K: int, data, weights, grad, loss, wr_
                                    _dev(wr_workspace, g.proj_shape(D), "wr_workspace"), _stream(stream)),
            "mm_loss_gradient")
     return grad, loss
+
+
+def mm_residual_loss(g: Geometry, B, vol, K: int, data, weights, wr, loss, stream=None):
+    import torch
+    ldk, D = vol.shape[-1], B.shape[-1]
+    w = ctypes.c_void_p(None) if weights is None else _dev(weights, g.proj_shape(D), "weights")
+    _check(load().mm_residual_loss(g._h, _dev(B, (g.P, K, D), "B"), _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, D,
+                                   _dev(data, g.proj_shape(D), "data"), w, _dev(wr, g.proj_shape(D), "wr"),
+                                   _dev(loss, (1,), "loss", torch.float64), _stream(stream)), "mm_residual_loss")
+    return wr, loss
+
+
+def mm_reciprocal(x, floor: float, stream=None):
+    _check(load().mm_reciprocal(_dev(x, x.shape, "x"), x.numel(), float(floor), _stream(stream)), "mm_reciprocal")
+    return x
+
+
+def mm_axpy_precond(c, grad, pre, eta: float, stream=None):
+    _check(load().mm_axpy_precond(_dev(c, c.shape, "c"), _dev(grad, c.shape, "grad"), _dev(pre, c.shape, "pre"), float(eta),
+                                  c.numel(), _stream(stream)), "mm_axpy_precond")
+    return c
 
 
 def mm_axpy(c, grad, eta: float, stream=None):

@@ -416,3 +416,43 @@ def test_tensor_core_adjoint_instantiations(ora, mm, K, ldk, D, P):
     c = Case((19, 17, 21), (24, 22), r.uniform(0, 2 * math.pi, P), r.uniform(-0.75, 0.75, P), K, ldk, D, seed=K + D,
              joff=r.uniform(-1, 1, P), koff=r.uniform(-1, 1, P))
     assert_errs(run_all_ops(ora, mm, c))
+
+
+@pytest.mark.parametrize("matched", [False, True])
+def test_sirt_iterations(ora, mm, matched):
+    """SIRT/MITRA as preconditioned weighted least squares (reading S19), composed from the C-ABI
+    calls: W = 1/(|A| 1), C = 1/(|A|' 1) by mm_forward / back-projector on ones + mm_reciprocal, then per iteration
+    mm_residual_loss -> mm_backproject (the paper's pair) or mm_adjoint (matched pair) -> mm_axpy_precond."""
+    import torch
+    cfg, c = cfg_case("C2", (22, 20, 24), (26, 25), 3, seed=31, joff=True, weights=None)
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    data = synth.poisson_data(ora.forward(go, B, c.vol[..., :K]), cfg.counts, cfg.seed)
+    W_o, C_o = ora.sirt_preconditioners(go, B, matched=matched)
+    back = mm.mm_adjoint if matched else mm.mm_backproject
+    dB, dabsB, dd = dev(B), dev(np.abs(B)), dev(data)
+    W = torch.empty(gm.proj_shape(D), device="cuda")
+    ones_v = torch.ones(gm.vol_shape(ldk), device="cuda")
+    mm.mm_forward(gm, dabsB, ones_v, K, W)
+    mm.mm_reciprocal(W, 1e-6)
+    Cp = torch.empty(gm.vol_shape(ldk), device="cuda")
+    back(gm, dabsB, torch.ones(gm.proj_shape(D), device="cuda"), K, Cp)
+    mm.mm_reciprocal(Cp, 1e-6)
+    assert einf(W.cpu().numpy(), W_o) <= TOL and einf(Cp.cpu().numpy()[..., :K], C_o) <= TOL
+    x_g = torch.zeros(gm.vol_shape(ldk), device="cuda")
+    x_o = np.zeros(c.shape + (K,), dtype=np.float32)
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    bp = torch.empty_like(x_g)
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    losses = []
+    for it in range(4):
+        mm.mm_residual_loss(gm, dB, x_g, K, dd, W, wr, loss)
+        back(gm, dB, wr, K, bp)
+        mm.mm_axpy_precond(x_g, bp, Cp, 1.0)
+        x_new, L_o = ora.sirt_step(go, B, x_o, data, W_o, C_o, matched=matched)
+        assert abs(loss.item() - L_o) <= TOL_LOSS * abs(L_o)
+        losses.append(L_o)
+        x_o = x_new.astype(np.float32)
+    assert einf(x_g.cpu().numpy()[..., :K], x_o) <= 1e-4            # errors compound over the iterations
+    assert losses[-1] < losses[0]
