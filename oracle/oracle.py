@@ -11,6 +11,7 @@ What is here (numpy, fp64) and what it follows:
   forward / adjoint    A = (basis map) o (John transform), Eq. 6-8, and A^T
   loss_gradient        r = Ac - I (Eq. 13), L = 1/2 sum w r^2, grad = A^T (w r)     PAPER.md:101, 324, readings S10, S11
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
+  basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
   sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
 
@@ -378,3 +379,40 @@ def sirt_step(g: Geometry, B, vol, data, W, C, matched=False, threads=None):
     wr = W * r
     back = adjoint(g, B, wr, form="scatter") if matched else backproject_bilinear(g, B, wr, threads)
     return np.asarray(vol, dtype=np.float64) - C * back, 0.5 * float(np.sum(wr * r))
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-2: basis sets defined by a grid of orientations
+# ------------------------------------------------------------------------------------------------
+def basis_matrix_grid(g: Geometry, dirs, kind, seg_start, seg_end, sigma=None, n_quad=16):
+    """B[P][K][D] float64 for the K basis functions attached to the unit vectors dirs[K][3] (sample frame):
+      kind "nn"  nearest-neighbour indicator functions: B_i(q) = 1 if g_i is the grid direction
+                 closest to the line through q (largest |q.g_i|, lowest index on ties), else 0;
+      kind "gk"  Gaussian kernels ("Bunge normal distribution"): B_i(q) = exp(-theta_i^2 / (2 sigma^2)),
+                 theta_i = arccos|q.g_i| the angle between the lines through q and g_i (reading S20: the RSM of
+                 SAXS is even in q, so distances are between lines, not vectors).
+    Eq. 3 (PAPER.md:60-68) by the midpoint rule with n_quad points per segment ("standard quadrature", PAPER.md:68;
+    n_quad = 1 is the central-angle approximation of PAPER.md:316)."""
+    dirs = np.asarray(dirs, dtype=np.float64)
+    dirs = dirs / np.linalg.norm(dirs, axis=1, keepdims=True)
+    seg_start = np.asarray(seg_start, dtype=np.float64)
+    seg_end = np.asarray(seg_end, dtype=np.float64)
+    K, D = dirs.shape[0], seg_start.size
+    B = np.zeros((g.P, K, D), dtype=np.float64)
+    t = (np.arange(n_quad) + 0.5) / n_quad
+    for s in range(g.P):
+        Rt = g.rotation_matrix(s).T
+        for c in range(D):
+            phi = seg_start[c] + (seg_end[c] - seg_start[c]) * t
+            qs = q_hat(g, phi) @ Rt.T                                  # rows R_s^T q(phi)
+            cosang = np.abs(qs @ dirs.T)                               # [n_quad][K]
+            if kind == "nn":
+                hit = np.zeros_like(cosang)
+                hit[np.arange(n_quad), np.argmax(cosang, axis=1)] = 1.0
+                B[s, :, c] = hit.mean(axis=0)
+            elif kind == "gk":
+                theta = np.arccos(np.minimum(cosang, 1.0))
+                B[s, :, c] = np.exp(-theta ** 2 / (2.0 * sigma ** 2)).mean(axis=0)
+            else:
+                raise ValueError(kind)
+    return B
