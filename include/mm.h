@@ -96,6 +96,17 @@ mm_status mm_geometry_get(const mm_geometry *g, int32_t s, double d[3], double j
 mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, int32_t D, const double *seg_start,
                              const double *seg_end, float *h_B);
 
+/* NEXT-2 — HOST helper, Eq. 3 for basis sets defined by a grid of orientations: dirs [n_dirs][3] HOST,
+ * sample-frame vectors (normalised here); K = n_dirs.
+ *   MM_BASIS_NN  nearest-neighbour indicators: B_i(q) = 1 if |q.g_i| is the largest (first on ties), else 0
+ *   MM_BASIS_GK  Gaussian kernels: B_i(q) = exp(-theta_i^2 / (2 sigma^2)), theta_i = arccos|q.g_i|
+ * (distances between lines, the SAXS RSM being even in q: DESIGN.md reading S20).  h_B[s][i][c] = mean of
+ * B_i(R_s^T q(phi)) over n_quad midpoints of [seg_start[c], seg_end[c]].  h_B [P][n_dirs][D] fp32 HOST. */
+#define MM_BASIS_NN 1
+#define MM_BASIS_GK 2
+mm_status mm_basis_grid_matrix(const mm_geometry *g, int32_t kind, int32_t n_dirs, const double *dirs, double sigma,
+                               int32_t D, const double *seg_start, const double *seg_end, int32_t n_quad, float *h_B);
+
 /* John transform, Eq. 5 / P:314, ray-stationary Joseph: for every ray (s,j,k) and channel i < K
  *   proj[s][j][k][i] = w_s * sum_{n=0}^{N_m-1} bilinear(vol[slab n])(pu_n, pv_n)_i, zero outside the volume.
  * vol [X][Y][Z][ldk] DEVICE in; proj [P][J][Kd][ldk] DEVICE out. */

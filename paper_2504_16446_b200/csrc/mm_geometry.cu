@@ -306,3 +306,55 @@ extern "C" mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, i
     }
     return MM_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-2: basis sets attached to a grid of orientations: nearest-neighbour indicators and
+// Gaussian kernels.  Same Eq. 3 segment average, midpoint rule with n_quad points (reading S20).
+// ------------------------------------------------------------------------------------------------
+extern "C" mm_status mm_basis_grid_matrix(const mm_geometry *g, int32_t kind, int32_t n_dirs, const double *dirs, double sigma,
+                                          int32_t D, const double *seg_start, const double *seg_end, int32_t n_quad, float *h_B)
+{
+    if (!g || !dirs || !seg_start || !seg_end || !h_B) { mm_set_error("mm_basis_grid_matrix: NULL argument"); return MM_ERR_NULL; }
+    if (n_dirs < 1 || D < 1 || n_quad < 1) { mm_set_error("mm_basis_grid_matrix: need n_dirs, D, n_quad >= 1"); return MM_ERR_SHAPE; }
+    if (kind != MM_BASIS_NN && kind != MM_BASIS_GK) { mm_set_error("mm_basis_grid_matrix: kind must be MM_BASIS_NN or MM_BASIS_GK"); return MM_ERR_VALUE; }
+    if (kind == MM_BASIS_GK && !(sigma > 0.0)) { mm_set_error("mm_basis_grid_matrix: sigma must be positive"); return MM_ERR_VALUE; }
+    std::vector<double> u((size_t)3 * n_dirs);                        // normalised grid directions
+    for (int i = 0; i < n_dirs; i++) {
+        const double *d = dirs + 3 * i;
+        const double n = sqrt(dot3(d, d));
+        if (!(n > 0.0) || !isfinite(n)) { mm_set_error("mm_basis_grid_matrix: zero or non-finite direction"); return MM_ERR_VALUE; }
+        for (int a = 0; a < 3; a++) u[3 * i + a] = d[a] / n;
+    }
+    std::vector<double> acc(n_dirs);
+    const double inv2s2 = kind == MM_BASIS_GK ? 0.5 / (sigma * sigma) : 0.0;
+    for (int s = 0; s < g->P; s++) {
+        const double *R = g->host[s].R;
+        for (int c = 0; c < D; c++) {
+            if (!isfinite(seg_start[c]) || !isfinite(seg_end[c])) { mm_set_error("non-finite segment angle"); return MM_ERR_VALUE; }
+            for (int i = 0; i < n_dirs; i++) acc[i] = 0.0;
+            for (int t = 0; t < n_quad; t++) {
+                const double phi = seg_start[c] + (seg_end[c] - seg_start[c]) * ((t + 0.5) / n_quad);
+                const double cp = cos(phi), sp = sin(phi);
+                double q[3], qs[3];
+                for (int a = 0; a < 3; a++) q[a] = cp * g->q0[a] + sp * g->q90[a];              // Eq. 1, small-angle line
+                for (int a = 0; a < 3; a++) qs[a] = R[a] * q[0] + R[3 + a] * q[1] + R[6 + a] * q[2];   // R_s^T q
+                if (kind == MM_BASIS_NN) {
+                    int best = 0;
+                    double bestc = -1.0;
+                    for (int i = 0; i < n_dirs; i++) {
+                        const double ca = fabs(dot3(qs, &u[3 * i]));
+                        if (ca > bestc) { bestc = ca; best = i; }                                // first maximum wins ties
+                    }
+                    acc[best] += 1.0;
+                } else {
+                    for (int i = 0; i < n_dirs; i++) {
+                        const double th = acos(fmin(fabs(dot3(qs, &u[3 * i])), 1.0));
+                        acc[i] += exp(-th * th * inv2s2);
+                    }
+                }
+            }
+            for (int i = 0; i < n_dirs; i++) h_B[((size_t)s * n_dirs + i) * D + c] = (float)(acc[i] / n_quad);
+        }
+    }
+    return MM_OK;
+}

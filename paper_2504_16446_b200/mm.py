@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm.so")
 _lib = None
 
-SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix",
+SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_residual_loss", "mm_reciprocal",
            "mm_axpy_precond", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
@@ -51,6 +51,7 @@ def load():
     L.mm_geometry_destroy.argtypes = [vp]
     L.mm_geometry_get.argtypes = [vp, i32, dp, dp, dp, ctypes.POINTER(i32), dp]
     L.mm_basis_sh_matrix.argtypes = [vp, i32, i32, dp, dp, vp]
+    L.mm_basis_grid_matrix.argtypes = [vp, i32, i32, dp, ctypes.c_double, i32, dp, dp, i32, vp]
     L.mm_john_forward.argtypes = [vp, vp, i32, i32, vp, vp]
     L.mm_john_adjoint.argtypes = [vp, vp, i32, i32, vp, vp]
     L.mm_basis_forward.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
@@ -165,6 +166,22 @@ def mm_basis_sh_matrix(g: Geometry, ell_max: int, seg_start, seg_end) -> np.ndar
     dp = ctypes.POINTER(ctypes.c_double)
     _check(load().mm_basis_sh_matrix(g._h, int(ell_max), D, s0.ctypes.data_as(dp), s1.ctypes.data_as(dp),
                                      ctypes.c_void_p(out.ctypes.data)), "mm_basis_sh_matrix")
+    return out
+
+
+MM_BASIS_NN, MM_BASIS_GK = 1, 2
+
+
+def mm_basis_grid_matrix(g: Geometry, kind: int, dirs, seg_start, seg_end, sigma: float = 0.0, n_quad: int = 16) -> np.ndarray:
+    """host helper: B[P][n_dirs][D] float32 (numpy) for the NN / GK basis set on the grid directions dirs[n][3]."""
+    d = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+    s0 = np.ascontiguousarray(seg_start, dtype=np.float64)
+    s1 = np.ascontiguousarray(seg_end, dtype=np.float64)
+    out = np.empty((g.P, d.shape[0], s0.size), dtype=np.float32)
+    dp = ctypes.POINTER(ctypes.c_double)
+    _check(load().mm_basis_grid_matrix(g._h, int(kind), d.shape[0], d.ctypes.data_as(dp), float(sigma), int(s0.size),
+                                       s0.ctypes.data_as(dp), s1.ctypes.data_as(dp), int(n_quad),
+                                       ctypes.c_void_p(out.ctypes.data)), "mm_basis_grid_matrix")
     return out
 
 

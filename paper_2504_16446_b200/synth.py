@@ -17,7 +17,7 @@ from dataclasses import dataclass, field, replace
 import numpy as np
 
 __all__ = ["Config", "CONFIGS", "get_config", "angles", "segments", "n_coeffs", "make_volume",
-           "make_weights", "poisson_data", "surrogate_model", "pad_channels", "ldk_for"]
+           "make_weights", "poisson_data", "surrogate_model", "pad_channels", "ldk_for", "grid_directions"]
 
 
 @dataclass(frozen=True)
@@ -274,6 +274,16 @@ def surrogate_model(cfg: Config, level: float = 1.0) -> np.ndarray:
     mod = 1.0 + 0.3 * np.cos(2.0 * (math.pi * (c[None, :] + 0.5) / cfg.D - 0.05 * s[:, None]))
     out = level * shadow[None, :, :, None] * mod[:, None, None, :].astype(np.float32)
     return np.ascontiguousarray(out, dtype=np.float32)
+
+
+def grid_directions(n: int) -> np.ndarray:
+    """n unit vectors spread over the upper half sphere (Fibonacci spiral) — a stand-in for the orientation grid
+    that defines an NN or GK basis set (the grid is an input of the method)."""
+    i = np.arange(n) + 0.5
+    z = i / n
+    ph = i * math.pi * (3.0 - math.sqrt(5.0))
+    rr = np.sqrt(1.0 - z * z)
+    return np.stack([rr * np.cos(ph), rr * np.sin(ph), z], axis=1)
 
 
 def pad_channels(a: np.ndarray, ldk: int) -> np.ndarray:

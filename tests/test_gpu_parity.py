@@ -456,3 +456,17 @@ def test_sirt_iterations(ora, mm, matched):
         x_o = x_new.astype(np.float32)
     assert einf(x_g.cpu().numpy()[..., :K], x_o) <= 1e-4            # errors compound over the iterations
     assert losses[-1] < losses[0]
+
+
+@pytest.mark.parametrize("kind,K", [("gk", 18), ("nn", 18), ("gk", 50)])
+def test_grid_basis_sets_through_the_same_kernels(ora, mm, kind, K):
+    """NEXT-2: GK / NN basis sets only change the B matrix; every device call is checked with
+    B built by the library's helper (K = 18 and 50 as in the paper's Table V; ldk 20 and 52)."""
+    r = np.random.default_rng(K)
+    P = 10
+    ldk = synth.ldk_for(K)
+    c = Case((18, 16, 20), (22, 21), r.uniform(0, 2 * math.pi, P), r.uniform(-0.7, 0.7, P), K, ldk, 8, seed=K)
+    _, gm = c.geoms(ora, mm)
+    c.B = mm.mm_basis_grid_matrix(gm, mm.MM_BASIS_GK if kind == "gk" else mm.MM_BASIS_NN, synth.grid_directions(K),
+                                  *synth.segments(8), sigma=0.3, n_quad=8)
+    assert_errs(run_all_ops(ora, mm, c))

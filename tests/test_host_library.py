@@ -136,3 +136,37 @@ def test_device_calls_fail_loudly_without_gpu(mm):
     st = L.mm_loss_gradient(g._h, dummy, dummy, 4, 4, 4, dummy, None, dummy, dummy, dummy, None)
     assert st == 5
     assert L.mm_launch_count() == 0
+
+
+@pytest.mark.parametrize("kind,name,sigma", [(1, "nn", 0.0), (2, "gk", 0.35)])
+def test_grid_basis_matrix_matches_oracle(mm, ora, kind, name, sigma):
+    """NEXT-2: the library's NN / GK basis-matrix helper against the oracle's (independent code, same quadrature)."""
+    from paper_2504_16446_b200 import synth
+    r = np.random.default_rng(17)
+    P = 11
+    rot, tilt = r.uniform(0, 2 * math.pi, P), r.uniform(-0.7, 0.7, P)
+    gm = mm.Geometry((5, 6, 7), (6, 5), rot, tilt)
+    go = ora.Geometry((5, 6, 7), (6, 5), rot, tilt)
+    dirs = synth.grid_directions(18) * r.uniform(0.5, 2.0, (18, 1))      # the helper normalises
+    s0, s1 = _segs(8)
+    got = mm.mm_basis_grid_matrix(gm, kind, dirs, s0, s1, sigma=sigma, n_quad=12)
+    want = ora.basis_matrix_grid(go, dirs, name, s0, s1, sigma=sigma or None, n_quad=12)
+    assert got.shape == want.shape == (P, 18, 8)
+    if name == "nn":
+        # an indicator can flip where two directions are equidistant to 1e-16: allow one quadrature point in a few entries
+        diff = np.abs(got - want)
+        assert diff.max() <= 1.0 / 12 + 1e-6 and (diff > 1e-6).mean() < 0.01
+        assert np.allclose(got.sum(axis=1), 1.0, atol=1e-6)
+    else:
+        assert np.abs(got - want).max() < 1e-6
+
+
+def test_grid_basis_matrix_rejects_bad_arguments(mm):
+    gm = mm.Geometry((4, 4, 4), (4, 4), [0.0], [0.0])
+    s0, s1 = _segs(4)
+    with pytest.raises(mm.MMError):
+        mm.mm_basis_grid_matrix(gm, 2, np.eye(3), s0, s1, sigma=0.0)          # GK needs sigma > 0
+    with pytest.raises(mm.MMError):
+        mm.mm_basis_grid_matrix(gm, 7, np.eye(3), s0, s1, sigma=1.0)          # unknown kind
+    with pytest.raises(mm.MMError):
+        mm.mm_basis_grid_matrix(gm, 1, np.zeros((2, 3)), s0, s1)              # zero direction
