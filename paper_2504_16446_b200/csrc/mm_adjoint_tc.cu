@@ -295,8 +295,8 @@ __device__ __forceinline__ void gather_voxel_bilinear(const TcProj &pg, const fl
 // two regions of ACCW columns each: the MMA accumulator of the current window, and the running sum
 template <int NPAD>
 struct TcCols {
-    static constexpr int accw = NPAD <= 16 ? 16 : (NPAD <= 32 ? 32 : 64);
-    static constexpr int value = 2 * accw < 32 ? 32 : 2 * accw;
+    static constexpr int accw = NPAD <= 16 ? 16 : (NPAD <= 32 ? 32 : (NPAD <= 64 ? 64 : (NPAD <= 128 ? 128 : 256)));
+    static constexpr int value = 2 * accw < 32 ? 32 : 2 * accw;      // a power of two, at most 512
 };
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -348,40 +348,45 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
         // groups are spread over the 32 lanes.  The global loads for chunk ch+1 are issued before this warp
         // waits for chunk ch's rows, so their latency is off the MMA's critical path.
         constexpr int BG = (NPAD * (KC / 4) + 31) / 32;       // groups per lane
-        float4 breg[BG];
-        auto load_b = [&](int s0) {
-#pragma unroll
-            for (int i = 0; i < BG; i++) {
-                const int g = lane + 32 * i;
-                const int n = g % NPAD, kg = g / NPAD;                // 16-byte group: columns 4kg .. 4kg+3
-                const int p = (4 * kg) / D, c = (4 * kg) % D, s = s0 + p;
-                float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (g < NPAD * (KC / 4) && n < a.K && s < a.P) {
-                    b = __ldg(reinterpret_cast<const float4 *>(a.B + ((long long)s * a.K + n) * D + c));
-                    const float w = __ldg(&a.tab[s].w);
-                    b.x *= w; b.y *= w; b.z *= w; b.w *= w;
-                }
-                breg[i] = b;
+        constexpr bool PREFETCH_B = BG <= 8;                  // wide accumulators: load B in place instead
+        float4 breg[PREFETCH_B ? BG : 1];
+        auto fetch_b = [&](int g, int s0) -> float4 {
+            const int n = g % NPAD, kg = g / NPAD;                    // 16-byte group: columns 4kg .. 4kg+3
+            const int p = (4 * kg) / D, c = (4 * kg) % D, s = s0 + p;
+            float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (g < NPAD * (KC / 4) && n < a.K && s < a.P) {
+                b = __ldg(reinterpret_cast<const float4 *>(a.B + ((long long)s * a.K + n) * D + c));
+                const float w = __ldg(&a.tab[s].w);
+                b.x *= w; b.y *= w; b.z *= w; b.w *= w;
             }
+            return b;
         };
-        load_b(0);
+        auto store_b = [&](int g, const float4 &b, float *Bhi, float *Blo) {
+            const int n = g % NPAD, kg = g / NPAD;
+            float4 h, l;
+            split_tf32(b.x, h.x, l.x); split_tf32(b.y, h.y, l.y); split_tf32(b.z, h.z, l.z); split_tf32(b.w, h.w, l.w);
+            *reinterpret_cast<float4 *>(Bhi + kg * (NPAD * 4) + n * 4) = h;
+            *reinterpret_cast<float4 *>(Blo + kg * (NPAD * 4) + n * 4) = l;
+        };
+        if constexpr (PREFETCH_B) {
+#pragma unroll
+            for (int i = 0; i < BG; i++) breg[i] = fetch_b(lane + 32 * i, 0);
+        }
         for (int ch = 0; ch < nch; ch++) {
             const int st = ch & 1;
             if (ch >= 2) mbar_wait(&empty[st], (uint32_t)(((ch >> 1) - 1) & 1));
             float *Bhi = sB + (2 * st) * B_FLOATS, *Blo = Bhi + B_FLOATS;
+            if constexpr (PREFETCH_B) {
 #pragma unroll
-            for (int i = 0; i < BG; i++) {
-                const int g = lane + 32 * i;
-                if (g < NPAD * (KC / 4)) {
-                    const int n = g % NPAD, kg = g / NPAD;
-                    const float4 b = breg[i];
-                    float4 h, l;
-                    split_tf32(b.x, h.x, l.x); split_tf32(b.y, h.y, l.y); split_tf32(b.z, h.z, l.z); split_tf32(b.w, h.w, l.w);
-                    *reinterpret_cast<float4 *>(Bhi + kg * (NPAD * 4) + n * 4) = h;
-                    *reinterpret_cast<float4 *>(Blo + kg * (NPAD * 4) + n * 4) = l;
+                for (int i = 0; i < BG; i++)
+                    if (lane + 32 * i < NPAD * (KC / 4)) store_b(lane + 32 * i, breg[i], Bhi, Blo);
+                if (ch + 1 < nch) {
+#pragma unroll
+                    for (int i = 0; i < BG; i++) breg[i] = fetch_b(lane + 32 * i, (ch + 1) * NPC);
                 }
+            } else {
+                for (int g = lane; g < NPAD * (KC / 4); g += 32) store_b(g, fetch_b(g, ch * NPC), Bhi, Blo);
             }
-            if (ch + 1 < nch) load_b((ch + 1) * NPC);
             fence_async_smem();
             __syncwarp();
             if (lane == 0) {
@@ -527,7 +532,7 @@ cudaError_t launch_tc(const AdjArgs &a, cudaStream_t st)
 
 bool mm_adjoint_tc_supported(const AdjArgs &a)
 {
-    return a.vec_ok && (a.D == 8 || a.D == 16) && a.ldk % 4 == 0 && a.ldk <= 64 &&
+    return a.vec_ok && (a.D == 8 || a.D == 16) && a.ldk % 4 == 0 && a.ldk <= 256 &&
            (long long)a.J * a.Kd * a.D < (1LL << 31) &&
            (reinterpret_cast<uintptr_t>(a.B) & 15u) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0 &&
            (reinterpret_cast<uintptr_t>(a.src) & 31u) == 0;      // 256-bit gather loads
@@ -536,15 +541,14 @@ bool mm_adjoint_tc_supported(const AdjArgs &a)
 int mm_adjoint_tc_launch(const AdjArgs &a, void *stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
-    const int npad = (a.ldk + 15) / 16 * 16;
-    if (a.D == 8) {
-        if (npad == 16) return launch_tc<8, 16>(a, st);
-        if (npad == 32) return launch_tc<8, 32>(a, st);
-        if (npad == 48) return launch_tc<8, 48>(a, st);
-        return launch_tc<8, 64>(a, st);
-    }
-    if (npad == 16) return launch_tc<16, 16>(a, st);
-    if (npad == 32) return launch_tc<16, 32>(a, st);
-    if (npad == 48) return launch_tc<16, 48>(a, st);
-    return launch_tc<16, 64>(a, st);
+    // accumulator width: the smallest instantiated multiple of 16 that holds ldk channels
+    const int w = a.ldk <= 16 ? 16 : a.ldk <= 32 ? 32 : a.ldk <= 48 ? 48 : a.ldk <= 64 ? 64 : a.ldk <= 96 ? 96 : a.ldk <= 128 ? 128
+                : a.ldk <= 192 ? 192 : 256;
+#define MM_TC_CASE(DD, NN) if (a.D == DD && w == NN) return launch_tc<DD, NN>(a, st)
+    MM_TC_CASE(8, 16); MM_TC_CASE(8, 32); MM_TC_CASE(8, 48); MM_TC_CASE(8, 64);
+    MM_TC_CASE(8, 96); MM_TC_CASE(8, 128); MM_TC_CASE(8, 192); MM_TC_CASE(8, 256);
+    MM_TC_CASE(16, 16); MM_TC_CASE(16, 32); MM_TC_CASE(16, 48); MM_TC_CASE(16, 64);
+    MM_TC_CASE(16, 96); MM_TC_CASE(16, 128); MM_TC_CASE(16, 192); MM_TC_CASE(16, 256);
+#undef MM_TC_CASE
+    return cudaErrorInvalidValue;
 }

@@ -408,7 +408,8 @@ def test_c5_full_size_sampled(ora, mm):
 
 
 @pytest.mark.parametrize("K,ldk,D,P", [(13, 16, 8, 7), (13, 16, 16, 5), (30, 32, 8, 19), (45, 48, 16, 9), (60, 64, 8, 17),
-                                        (61, 64, 16, 33)])
+                                        (61, 64, 16, 33), (90, 92, 8, 9), (120, 128, 16, 7), (162, 164, 8, 11),
+                                        (250, 252, 8, 5), (200, 200, 16, 4)])
 def test_tensor_core_adjoint_instantiations(ora, mm, K, ldk, D, P):
     """every (D, accumulator width) instantiation of the tcgen05 adjoint, with projection counts that leave a
     short last chunk (P odd), fewer chunks than one accumulation window, and more than two windows."""
