@@ -12,6 +12,7 @@ What is here (numpy, fp64) and what it follows:
   loss_gradient        r = Ac - I (Eq. 13), L = 1/2 sum w r^2, grad = A^T (w r)     PAPER.md:101, 324, readings S10, S11
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
   basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
+  laplacian / laplacian_regulariser / l2_regulariser / nesterov_step   regularisers, momentum   PAPER.md:336-340 (NEXT-3)
   sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
 
@@ -416,3 +417,40 @@ def basis_matrix_grid(g: Geometry, dirs, kind, seg_start, seg_end, sigma=None, n
             else:
                 raise ValueError(kind)
     return B
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: regulariser gradients and momentum
+# ------------------------------------------------------------------------------------------------
+def laplacian(vol):
+    """finite-difference Laplacian of every channel of vol[X][Y][Z][K] ("finite-difference Laplacian
+    operator of the tensor field"): 7-point stencil, unit spacing, neighbours outside the volume count as 0
+    (reading S21: the paper does not state the boundary rule; zero padding is the one the forward model uses)."""
+    v = np.asarray(vol, dtype=np.float64)
+    out = -6.0 * v
+    for ax in range(3):
+        lo = [slice(None)] * 4
+        hi = [slice(None)] * 4
+        lo[ax], hi[ax] = slice(0, -1), slice(1, None)
+        out[tuple(lo)] += v[tuple(hi)]
+        out[tuple(hi)] += v[tuple(lo)]
+    return out
+
+
+def laplacian_regulariser(vol):
+    """(R, grad): R = 1/2 ||Lap c||^2, grad = Lap^T Lap c = Lap(Lap c) (the zero-padded stencil is symmetric)."""
+    l = laplacian(vol)
+    return 0.5 * float(np.sum(l * l)), laplacian(l)
+
+
+def l2_regulariser(vol):
+    """(R, grad) of the L2Norm regulariser: R = 1/2 ||c||^2, grad = c."""
+    v = np.asarray(vol, dtype=np.float64)
+    return 0.5 * float(np.sum(v * v)), v.copy()
+
+
+def nesterov_step(c, v, grad_at_lookahead, eta, momentum):
+    """GradientDescent with Nesterov accelerated momentum; reading S22, the usual form:
+        v <- m v - eta g(c + m v);   c <- c + v.   Returns (c_new, v_new); the caller evaluates g at c + m v."""
+    v_new = momentum * np.asarray(v, dtype=np.float64) - eta * np.asarray(grad_at_lookahead, dtype=np.float64)
+    return np.asarray(c, dtype=np.float64) + v_new, v_new
