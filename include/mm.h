@@ -170,6 +170,16 @@ mm_status mm_residual_loss(const mm_geometry *g, const float *B, const float *vo
 mm_status mm_reciprocal(float *x, int64_t n, float floor, void *stream);
 mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float eta, int64_t n, void *stream);
 
+/* NEXT-3 — regulariser and optimizer building blocks for a device-resident iteration.
+ * mm_laplacian: vol_out[x][i] = sum of the six face neighbours of vol[x][i] - 6 vol[x][i], neighbours outside the
+ *   volume counting as 0 (reading S21); vol, vol_out [X][Y][Z][ldk] DEVICE, distinct; pad channels written 0.
+ *   The gradient of the Laplacian regulariser mu/2 ||Lap c||^2 is mu Lap(Lap c): two calls; of the L2Norm
+ *   mu/2 ||c||^2 it is mu c: mm_axpy(grad, c, -mu, n).
+ * mm_nesterov_step: v <- momentum v - eta grad;  c <- c + v  (GradientDescent with Nesterov momentum; the
+ *   caller evaluates grad at c + momentum v, reading S22); n floats each, DEVICE. */
+mm_status mm_laplacian(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *vol_out, void *stream);
+mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream);
+
 /* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */
 mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream);
 

@@ -577,6 +577,49 @@ __global__ void reciprocal_kernel(float *__restrict__ x, float floor_, long long
     if (i < n) { const float v = x[i]; x[i] = v > floor_ ? 1.f / v : 0.f; }
 }
 
+// NEXT-3: zero-padded 7-point Laplacian of every channel; one thread per float4 of the volume,
+// neighbours along z are adjacent records, along y and x one row / plane away (all coalesced 16-byte loads)
+template <int VEC>
+__global__ void laplacian_kernel(const float *__restrict__ in, float *__restrict__ out, int X, int Y, int Z, int ldk, int K)
+{
+    const int lpv = ldk / VEC;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)X * Y * Z * lpv;
+    if (idx >= total) return;
+    const int e = (int)(idx % lpv);
+    const long long vox = idx / lpv;
+    const int z = (int)(vox % Z), y = (int)((vox / Z) % Y), x = (int)(vox / ((long long)Z * Y));
+    const long long sZ = ldk, sY = (long long)Z * ldk, sX = (long long)Y * Z * ldk;
+    const float *p = in + vox * ldk + VEC * e;
+    float c[VEC], acc[VEC], nb[VEC];
+    Ld<VEC>::ld(p, c);
+#pragma unroll
+    for (int i = 0; i < VEC; i++) acc[i] = -6.f * c[i];
+#define MM_LAP_TAP(cond, off)                                    \
+    if (cond) {                                                  \
+        Ld<VEC>::ld(p + (off), nb);                              \
+        _Pragma("unroll") for (int i = 0; i < VEC; i++) acc[i] += nb[i]; \
+    }
+    MM_LAP_TAP(z > 0, -sZ) MM_LAP_TAP(z + 1 < Z, sZ)
+    MM_LAP_TAP(y > 0, -sY) MM_LAP_TAP(y + 1 < Y, sY)
+    MM_LAP_TAP(x > 0, -sX) MM_LAP_TAP(x + 1 < X, sX)
+#undef MM_LAP_TAP
+#pragma unroll
+    for (int i = 0; i < VEC; i++) acc[i] = (VEC * e + i < K) ? acc[i] : 0.f;
+    Ld<VEC>::st(out + vox * ldk + VEC * e, acc);
+}
+
+// Nesterov momentum (reading S22): v <- m v - eta g;  c <- c + v
+__global__ void nesterov_kernel(float *__restrict__ c, float *__restrict__ v, const float *__restrict__ g, float eta, float m, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        const float vn = fmaf(m, v[i], -eta * g[i]);
+        v[i] = vn;
+        c[i] += vn;
+    }
+}
+
 // preconditioned update c <- c - eta * pre (.) g
 __global__ void axpy_precond_kernel(float *__restrict__ c, const float *__restrict__ g, const float *__restrict__ pre, float eta, long long n)
 {
@@ -870,6 +913,30 @@ extern "C" mm_status mm_reciprocal(float *x, int64_t n, float floor_, void *stre
     if (n == 0) return MM_OK;
     reciprocal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, floor_, (long long)n);
     return check_launch("reciprocal_kernel");
+}
+
+extern "C" mm_status mm_laplacian(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *vol_out, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_laplacian");
+    if (st != MM_OK) return st;
+    if (!vol || !vol_out) { mm_set_error("mm_laplacian: NULL buffer"); return MM_ERR_NULL; }
+    if (vol == vol_out) { mm_set_error("mm_laplacian: in and out must differ"); return MM_ERR_VALUE; }
+    const int X = g->shape[0], Y = g->shape[1], Z = g->shape[2];
+    const bool vec = (ldk % 4 == 0) && aligned16(vol) && aligned16(vol_out);
+    const long long total = (long long)X * Y * Z * (vec ? ldk / 4 : ldk);
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (vec) laplacian_kernel<4><<<blocks, 256, 0, (cudaStream_t)stream>>>(vol, vol_out, X, Y, Z, ldk, K);
+    else laplacian_kernel<1><<<blocks, 256, 0, (cudaStream_t)stream>>>(vol, vol_out, X, Y, Z, ldk, K);
+    return check_launch("laplacian_kernel");
+}
+
+extern "C" mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream)
+{
+    if (!c || !v || !grad) { mm_set_error("mm_nesterov_step: NULL buffer"); return MM_ERR_NULL; }
+    if (n < 0) { mm_set_error("mm_nesterov_step: n < 0"); return MM_ERR_SHAPE; }
+    if (n == 0) return MM_OK;
+    nesterov_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(c, v, grad, eta, momentum, (long long)n);
+    return check_launch("nesterov_kernel");
 }
 
 extern "C" mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float eta, int64_t n, void *stream)

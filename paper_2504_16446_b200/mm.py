@@ -19,7 +19,7 @@ _lib = None
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_residual_loss", "mm_reciprocal",
-           "mm_axpy_precond", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
+           "mm_axpy_precond", "mm_laplacian", "mm_nesterov_step", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -64,6 +64,8 @@ def load():
     L.mm_axpy.argtypes = [vp, vp, ctypes.c_float, i64, vp]
     L.mm_residual_loss.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.mm_reciprocal.argtypes = [vp, i64, ctypes.c_float, vp]
+    L.mm_laplacian.argtypes = [vp, vp, i32, i32, vp, vp]
+    L.mm_nesterov_step.argtypes = [vp, vp, vp, ctypes.c_float, ctypes.c_float, i64, vp]
     L.mm_axpy_precond.argtypes = [vp, vp, vp, ctypes.c_float, i64, vp]
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
     L.mm_set_phase_event.argtypes = [vp]
@@ -273,6 +275,19 @@ def mm_axpy_precond(c, grad, pre, eta: float, stream=None):
     _check(load().mm_axpy_precond(_dev(c, c.shape, "c"), _dev(grad, c.shape, "grad"), _dev(pre, c.shape, "pre"), float(eta),
                                   c.numel(), _stream(stream)), "mm_axpy_precond")
     return c
+
+
+def mm_laplacian(g: Geometry, vol, K: int, vol_out, stream=None):
+    ldk = vol.shape[-1]
+    _check(load().mm_laplacian(g._h, _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, _dev(vol_out, g.vol_shape(ldk), "vol_out"),
+                               _stream(stream)), "mm_laplacian")
+    return vol_out
+
+
+def mm_nesterov_step(c, v, grad, eta: float, momentum: float, stream=None):
+    _check(load().mm_nesterov_step(_dev(c, c.shape, "c"), _dev(v, c.shape, "v"), _dev(grad, c.shape, "grad"), float(eta),
+                                   float(momentum), c.numel(), _stream(stream)), "mm_nesterov_step")
+    return c, v
 
 
 def mm_axpy(c, grad, eta: float, stream=None):

@@ -471,3 +471,54 @@ def test_grid_basis_sets_through_the_same_kernels(ora, mm, kind, K):
     c.B = mm.mm_basis_grid_matrix(gm, mm.MM_BASIS_GK if kind == "gk" else mm.MM_BASIS_NN, synth.grid_directions(K),
                                   *synth.segments(8), sigma=0.3, n_quad=8)
     assert_errs(run_all_ops(ora, mm, c))
+
+
+@pytest.mark.parametrize("K,ldk,shape", [(6, 8, (17, 13, 19)), (5, 5, (9, 1, 7)), (45, 48, (12, 14, 10)), (1, 1, (1, 1, 1))])
+def test_laplacian(ora, mm, K, ldk, shape):
+    """NEXT-3: zero-padded 7-point Laplacian of every channel (reading S21), float4 and scalar paths."""
+    import torch
+    gm = mm.Geometry(shape, (4, 4), [0.0], [0.0])
+    v = np.random.default_rng(K).standard_normal(shape + (ldk,)).astype(np.float32)
+    out = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    mm.mm_laplacian(gm, dev(v), K, out)
+    got = out.cpu().numpy()
+    want = ora.laplacian(v[..., :K])
+    assert np.abs(got[..., :K] - want).max() <= 1e-5 * max(1.0, np.abs(want).max()) and np.all(got[..., K:] == 0.0)
+
+
+def test_regularised_nesterov_iterations(ora, mm):
+    """a device-resident MITRA/SIGTT-style loop: data term + Laplacian + L2 regularisers,
+    Nesterov momentum, composed from the C-ABI calls; trajectory and losses against the oracle."""
+    import torch
+    cfg, c = cfg_case("C2", (18, 16, 20), (22, 21), 3, seed=41, weights=None)
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    data = synth.poisson_data(ora.forward(go, B, c.vol[..., :K]), cfg.counts, cfg.seed)
+    absB = np.abs(B)
+    lip = float(ora.forward(go, absB, np.ones(c.shape + (K,), np.float32)).max() *
+                ora.adjoint(go, absB, np.ones((c.P,) + c.det + (D,)), form="scatter").max())
+    mu_lap, mu_l2, mom = 1e-3 * lip, 1e-4 * lip, 0.8
+    eta = 1.0 / (lip + 144.0 * mu_lap + mu_l2)                       # ||Lap||^2 <= 12^2
+    dB, dd = dev(B), dev(data)
+    n = int(np.prod(gm.vol_shape(ldk)))
+    x = torch.zeros(gm.vol_shape(ldk), device="cuda"); v = torch.zeros_like(x)
+    look, grad, l1, l2 = (torch.empty_like(x) for _ in range(4))
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    x_o = np.zeros(c.shape + (K,)); v_o = np.zeros_like(x_o)
+    for it in range(4):
+        # look-ahead point c + m v (torch only moves memory here: a copy and the library's own axpy)
+        look.copy_(x); mm.mm_axpy(look, v, -mom)
+        mm.mm_loss_gradient(gm, dB, look, K, dd, None, grad, loss, wr)
+        mm.mm_laplacian(gm, look, K, l1); mm.mm_laplacian(gm, l1, K, l2)
+        mm.mm_axpy(grad, l2, -mu_lap); mm.mm_axpy(grad, look, -mu_l2)
+        mm.mm_nesterov_step(x, v, grad, eta, mom)
+        look_o = (x_o + np.float32(mom) * v_o).astype(np.float32)
+        L_o, g_o, _ = ora.loss_gradient(go, B, look_o, data, None, form="scatter")
+        g_o = g_o + np.float32(mu_lap) * ora.laplacian_regulariser(look_o)[1] + np.float32(mu_l2) * ora.l2_regulariser(look_o)[1]
+        x_o, v_o = ora.nesterov_step(x_o, v_o, g_o, np.float32(eta), np.float32(mom))
+        assert abs(loss.item() - L_o) <= TOL_LOSS * abs(L_o)
+        if it == 0:
+            assert einf(grad.cpu().numpy()[..., :K], g_o) <= TOL
+    assert einf(x.cpu().numpy()[..., :K], x_o) <= 1e-4 and einf(v.cpu().numpy()[..., :K], v_o) <= 1e-4
