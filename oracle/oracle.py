@@ -13,6 +13,7 @@ What is here (numpy, fp64) and what it follows:
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
   basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
   laplacian / laplacian_regulariser / l2_regulariser / nesterov_step   regularisers, momentum   PAPER.md:336-340 (NEXT-3)
+  huber_loss_gradient  Huber-regressor loss and its gradient   PAPER.md:334 (NEXT-4, reading S23)
   sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
 
@@ -454,3 +455,19 @@ def nesterov_step(c, v, grad_at_lookahead, eta, momentum):
         v <- m v - eta g(c + m v);   c <- c + v.   Returns (c_new, v_new); the caller evaluates g at c + m v."""
     v_new = momentum * np.asarray(v, dtype=np.float64) - eta * np.asarray(grad_at_lookahead, dtype=np.float64)
     return np.asarray(c, dtype=np.float64) + v_new, v_new
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: robust regression, PAPER.md:334 (HuberLoss)
+# ------------------------------------------------------------------------------------------------
+def huber_loss_gradient(g: Geometry, B, vol, data, delta, weights=None, form="gather", threads=None):
+    """Huber regressor on the residual r = A c - I (ref. 53; reading S23, the textbook form):
+        rho(r) = 1/2 r^2 if |r| <= delta, else delta (|r| - delta/2);   L = sum w rho(r);
+        grad = A^T (w psi(r)),  psi(r) = rho'(r) = clip(r, -delta, delta).
+    Returns (L, grad[X][Y][Z][K], w psi[P][J][Kd][D])."""
+    r = forward(g, B, vol, threads) - np.asarray(data, dtype=np.float64)
+    w = np.ones_like(r) if weights is None else np.asarray(weights, dtype=np.float64)
+    a = np.abs(r)
+    rho = np.where(a <= delta, 0.5 * r * r, delta * (a - 0.5 * delta))
+    wpsi = w * np.clip(r, -delta, delta)
+    return float(np.sum(w * rho)), adjoint(g, B, wpsi, form=form, threads=threads), wpsi

@@ -136,3 +136,28 @@ def test_forward_rays_matches_full(ora):
     I = ora.forward(g, B, vol)
     sjk = np.array([[0, 0, 0], [3, 6, 5], [2, 3, 3]], dtype=np.int32)
     assert np.abs(ora.forward_rays(g, B, vol, sjk) - I[sjk[:, 0], sjk[:, 1], sjk[:, 2]]).max() < 1e-13
+
+
+def test_huber_loss_limits_and_gradient(ora):
+    """NEXT-4: Huber = squared loss for delta above every |r|; linear growth delta(|r| - delta/2) far
+    out; gradient checked by finite differences (rho is C^1)."""
+    r = np.random.default_rng(12)
+    shape, det, P, K, D = (6, 5, 7), (8, 7), 4, 3, 4
+    g = ora.Geometry(shape, det, r.uniform(0, 6.28, P), r.uniform(-0.5, 0.5, P))
+    B = r.standard_normal((P, K, D))
+    c = r.standard_normal(shape + (K,)).astype(np.float32)
+    data = ora.forward(g, B, c) + r.standard_normal((P,) + det + (D,)) * 3.0
+    w = r.uniform(0.5, 1.5, (P,) + det + (D,))
+    L2, g2, wr2 = ora.loss_gradient(g, B, c, data, w)
+    Lh, gh, wpsi = ora.huber_loss_gradient(g, B, c, data, 1e9, w)
+    assert abs(Lh - L2) < 1e-9 * L2 and np.abs(gh - g2).max() < 1e-9 and np.abs(wpsi - wr2).max() < 1e-12
+    delta = 1.0
+    Lh, gh, wpsi = ora.huber_loss_gradient(g, B, c, data, delta, w)
+    res = ora.forward(g, B, c) - data
+    big = np.abs(res) > delta
+    assert big.any() and (~big).any() and np.abs(wpsi).max() <= 1.5 * delta + 1e-12
+    assert abs(Lh - (np.sum(w[~big] * 0.5 * res[~big] ** 2) + np.sum(w[big] * delta * (np.abs(res[big]) - 0.5 * delta)))) < 1e-9 * Lh
+    d = r.standard_normal(c.shape).astype(np.float32)
+    h = 1e-3
+    fd = (ora.huber_loss_gradient(g, B, c + h * d, data, delta, w)[0] - ora.huber_loss_gradient(g, B, c - h * d, data, delta, w)[0]) / (2 * h)
+    assert abs(fd - np.sum(gh * d)) < 2e-4 * abs(fd)
