@@ -157,6 +157,13 @@ mm_status mm_loss_gradient(const mm_geometry *g, const float *B, const float *vo
                            int32_t D, const float *data, const float *weights, float *grad, double *loss,
                            float *wr_workspace, void *stream);
 
+/* NEXT-4 — robust regression (HuberLoss; reading S23): as mm_loss_gradient with the Huber function of the
+ * residual, rho(r) = 1/2 r^2 for |r| <= delta, delta (|r| - delta/2) beyond:  *loss = sum weights rho(r),
+ * wr_workspace = weights * clip(r, -delta, delta), grad = A^T wr_workspace.  delta > 0. */
+mm_status mm_loss_gradient_huber(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                 const float *data, const float *weights, float delta, float *grad, double *loss,
+                                 float *wr_workspace, void *stream);
+
 /* Phase 1 of mm_loss_gradient alone: wr = weights * (A vol - data), *loss = 1/2 sum weights r^2; lets a caller
  * pair the forward with the back-projector of its choice (mm_adjoint or mm_backproject), as SIRT/MITRA do.
  * Same arguments as mm_loss_gradient; wr [P][J][Kd][D] DEVICE out. */

@@ -57,6 +57,7 @@ struct FwdArgs {
     const float *weights;     // MODE 2 (may be NULL)
     float *sino;              // MODE 1: model sinogram; MODE 2: wr
     double *loss;             // MODE 2
+    float huber;              // MODE 2: Huber threshold delta; <= 0 = squared loss
 };
 
 template <int VEC>
@@ -338,9 +339,14 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
             } else {
                 const float res = part[c] - __ldg(a.data + o);            // r = Ac - I  (Eq. 13)
                 const float wt = a.weights ? __ldg(a.weights + o) : 1.f;
-                const float wr = wt * res;
-                a.sino[o] = wr;
-                lsum += 0.5 * (double)wr * (double)res;                    // L = 1/2 sum w r^2  (S10)
+                float psi = res;                                           // rho'(r): r, or clip(r, -delta, delta) (Huber, S23)
+                double rho = 0.5 * (double)res * (double)res;             // L = sum w rho(r): 1/2 r^2 (S10) ...
+                if (a.huber > 0.f && fabsf(res) > a.huber) {
+                    psi = copysignf(a.huber, res);
+                    rho = (double)a.huber * ((double)fabsf(res) - 0.5 * (double)a.huber);   // ... or delta (|r| - delta/2)
+                }
+                a.sino[o] = wt * psi;
+                lsum += (double)wt * rho;
             }
         }
     }
@@ -704,6 +710,7 @@ void fill_fwd(FwdArgs &a, const mm_geometry *g, const float *vol, int K, int ldk
     a.tab = g->d_table; a.vol = vol; a.K = K; a.ldk = ldk;
     a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
     a.proj = nullptr; a.B = nullptr; a.D = 0; a.data = nullptr; a.weights = nullptr; a.sino = nullptr; a.loss = nullptr;
+    a.huber = 0.f;
 }
 
 void fill_adj(AdjArgs &a, const mm_geometry *g, const float *src, const float *B, float *out, int K, int ldk, int D)
@@ -868,7 +875,7 @@ extern "C" mm_status mm_basis_adjoint(const mm_geometry *g, const float *B, cons
 
 static mm_status run_residual_loss(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
                                    const float *data, const float *weights, float *wr, double *loss, cudaStream_t cs,
-                                   const char *who)
+                                   const char *who, float huber = 0.f)
 {
     mm_status st = check_common(g, K, ldk, who);
     if (st != MM_OK) return st;
@@ -880,7 +887,7 @@ static mm_status run_residual_loss(const mm_geometry *g, const float *B, const f
     }
     FwdArgs a;
     fill_fwd(a, g, vol, K, ldk);
-    a.B = B; a.D = D; a.data = data; a.weights = weights; a.sino = wr; a.loss = loss;
+    a.B = B; a.D = D; a.data = data; a.weights = weights; a.sino = wr; a.loss = loss; a.huber = huber;
     const bool vec = (ldk % 4 == 0) && aligned16(vol);
     return dispatch_fwd_d<2>(a, vec, cs);                     // a3 + a4 + a5
 }
@@ -904,6 +911,18 @@ extern "C" mm_status mm_loss_gradient(const mm_geometry *g, const float *B, cons
         return MM_ERR_CUDA;
     }
     return run_adjoint_fused(g, B, wr_workspace, K, ldk, D, grad, cs);   // phase 2: a6 + a7
+}
+
+extern "C" mm_status mm_loss_gradient_huber(const mm_geometry *g, const float *B, const float *vol, int32_t K, int32_t ldk, int32_t D,
+                                            const float *data, const float *weights, float delta, float *grad, double *loss,
+                                            float *wr_workspace, void *stream)
+{
+    if (!grad) { mm_set_error("mm_loss_gradient_huber: NULL buffer"); return MM_ERR_NULL; }
+    if (!(delta > 0.f)) { mm_set_error("mm_loss_gradient_huber: delta must be positive"); return MM_ERR_VALUE; }
+    cudaStream_t cs = (cudaStream_t)stream;
+    mm_status st = run_residual_loss(g, B, vol, K, ldk, D, data, weights, wr_workspace, loss, cs, "mm_loss_gradient_huber", delta);
+    if (st != MM_OK) return st;
+    return run_adjoint_fused(g, B, wr_workspace, K, ldk, D, grad, cs);
 }
 
 extern "C" mm_status mm_reciprocal(float *x, int64_t n, float floor_, void *stream)

@@ -18,7 +18,7 @@ _lib = None
 
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
-           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_residual_loss", "mm_reciprocal",
+           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
            "mm_axpy_precond", "mm_laplacian", "mm_nesterov_step", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
@@ -63,6 +63,7 @@ def load():
     L.mm_loss_gradient.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     L.mm_axpy.argtypes = [vp, vp, ctypes.c_float, i64, vp]
     L.mm_residual_loss.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp]
+    L.mm_loss_gradient_huber.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, ctypes.c_float, vp, vp, vp, vp]
     L.mm_reciprocal.argtypes = [vp, i64, ctypes.c_float, vp]
     L.mm_laplacian.argtypes = [vp, vp, i32, i32, vp, vp]
     L.mm_nesterov_step.argtypes = [vp, vp, vp, ctypes.c_float, ctypes.c_float, i64, vp]
@@ -253,6 +254,18 @@ def mm_loss_gradient(g: Geometry, B, vol, K: int, data, weights, grad, loss, wr_
                                    _dev(loss, (1,), "loss", torch.float64),
                                    _dev(wr_workspace, g.proj_shape(D), "wr_workspace"), _stream(stream)),
            "mm_loss_gradient")
+    return grad, loss
+
+
+def mm_loss_gradient_huber(g: Geometry, B, vol, K: int, data, weights, delta: float, grad, loss, wr_workspace, stream=None):
+    import torch
+    ldk, D = vol.shape[-1], B.shape[-1]
+    w = ctypes.c_void_p(None) if weights is None else _dev(weights, g.proj_shape(D), "weights")
+    _check(load().mm_loss_gradient_huber(g._h, _dev(B, (g.P, K, D), "B"), _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, D,
+                                         _dev(data, g.proj_shape(D), "data"), w, float(delta),
+                                         _dev(grad, g.vol_shape(ldk), "grad"), _dev(loss, (1,), "loss", torch.float64),
+                                         _dev(wr_workspace, g.proj_shape(D), "wr_workspace"), _stream(stream)),
+           "mm_loss_gradient_huber")
     return grad, loss
 
 

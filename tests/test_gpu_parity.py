@@ -522,3 +522,35 @@ def test_regularised_nesterov_iterations(ora, mm):
         if it == 0:
             assert einf(grad.cpu().numpy()[..., :K], g_o) <= TOL
     assert einf(x.cpu().numpy()[..., :K], x_o) <= 1e-4 and einf(v.cpu().numpy()[..., :K], v_o) <= 1e-4
+
+
+@pytest.mark.parametrize("weights", ["uniform", None])
+def test_huber_loss_gradient(ora, mm, weights):
+    """NEXT-4 (reading S23): Huber-regressor loss, clipped weighted residual and gradient; a threshold
+    that clips about a third of the residuals, and a huge one that must reproduce mm_loss_gradient bit for bit."""
+    import torch
+    cfg, c = cfg_case("C3", (20, 18, 22), (25, 24), 2, seed=51, joff=True, weights=weights)
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    model = ora.forward(go, B, c.vol[..., :K])
+    scale = float(np.abs(model).max())
+    data = (model + 0.05 * scale * c.data).astype(np.float32)
+    delta = 0.05 * scale                                            # |noise| > delta for ~32 % of the samples
+    dB, dvol, dd = dev(B), dev(c.vol), dev(data)
+    dw = None if c.w is None else dev(c.w)
+    grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    wr = torch.empty(gm.proj_shape(D), device="cuda")
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    mm.mm_loss_gradient_huber(gm, dB, dvol, K, dd, dw, delta, grad, loss, wr)
+    L, g_o, wpsi = ora.huber_loss_gradient(go, B, c.vol[..., :K], data, delta, c.w, form="scatter")
+    clipped = np.isclose(np.abs(wpsi), delta * (1.0 if c.w is None else c.w))
+    assert 0.15 < clipped.mean() < 0.5
+    assert abs(loss.item() - L) <= TOL_LOSS * L
+    assert np.abs(wr.cpu().numpy() - wpsi).max() / scale <= TOL
+    got = grad.cpu().numpy()
+    assert einf(got[..., :K], g_o) <= TOL and np.all(got[..., K:] == 0.0)
+    g2, wr2, loss2 = torch.empty_like(grad), torch.empty_like(wr), torch.zeros_like(loss)
+    mm.mm_loss_gradient_huber(gm, dB, dvol, K, dd, dw, 1e30, grad, loss, wr)
+    mm.mm_loss_gradient(gm, dB, dvol, K, dd, dw, g2, loss2, wr2)
+    assert torch.equal(grad, g2) and torch.equal(wr, wr2) and abs(loss.item() - loss2.item()) <= 1e-12 * loss2.item()
