@@ -249,13 +249,16 @@ def real_sh(l: int, m: int, n):
     return norm * plm
 
 
-def q_hat(g: Geometry, phi):
-    """lab-frame scattering direction, small-angle line of Eq. 1: cos(phi) q0 + sin(phi) q90."""
+def q_hat(g: Geometry, phi, two_theta=0.0):
+    """lab-frame scattering direction, Eq. 1:
+        q(phi) = cos(2theta/2) (cos(phi) q0 + sin(phi) q90) - sin(2theta/2) p;
+    two_theta = 0 is the small-angle second line, cos(phi) q0 + sin(phi) q90 (reading S13, the SAXS default)."""
     phi = np.asarray(phi, dtype=np.float64)
-    return np.cos(phi)[..., None] * g.vecs["q0"] + np.sin(phi)[..., None] * g.vecs["q90"]
+    inplane = np.cos(phi)[..., None] * g.vecs["q0"] + np.sin(phi)[..., None] * g.vecs["q90"]
+    return math.cos(0.5 * two_theta) * inplane - math.sin(0.5 * two_theta) * g.vecs["p"]
 
 
-def basis_matrix(g: Geometry, ell_max: int, seg_start, seg_end, n_quad: int = 32, rule: str = "gauss"):
+def basis_matrix(g: Geometry, ell_max: int, seg_start, seg_end, n_quad: int = 32, rule: str = "gauss", two_theta: float = 0.0):
     """B[P][K][D] float64: B[s][i][c] = mean over [start_c, end_c] of Y_i(R_s^T q(phi))  (Eq. 3).
     rule = 'gauss' (Gauss-Legendre, n_quad nodes), 'simpson' (composite, n_quad panels) or 'central'
     (the central-angle approximation the paper mentions)."""
@@ -281,7 +284,7 @@ def basis_matrix(g: Geometry, ell_max: int, seg_start, seg_end, n_quad: int = 32
         Rt = g.rotation_matrix(s).T
         for c in range(D):
             phi = 0.5 * (seg_start[c] + seg_end[c]) + 0.5 * (seg_end[c] - seg_start[c]) * xs
-            qs = q_hat(g, phi) @ Rt.T                   # rows: R_s^T q(phi)
+            qs = q_hat(g, phi, two_theta) @ Rt.T        # rows: R_s^T q(phi)
             for i, (l, m) in enumerate(idx):
                 B[s, i, c] = np.dot(ws, real_sh(l, m, qs))
     return B

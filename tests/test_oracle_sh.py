@@ -157,3 +157,27 @@ def test_B_rotation_covariance(ora):
             q = (np.cos(phi)[:, None] * g.vecs["q0"] + np.sin(phi)[:, None] * g.vecs["q90"]) @ Rt.T
             rhs = np.dot(ws / 2, (2 * l + 1) * leg.Legendre.basis(l)(q @ n))
             assert abs(lhs[c] - rhs) < 1e-11, (l, c)
+
+
+def test_full_two_theta_scattering_vector(ora):
+    """NEXT-4: first line of Eq. 1.  q stays a unit vector; 2theta = 0 is the small-angle line; with
+    R_s = 1 and p = z the z-component is -sin(theta) for every phi, so the segment average of
+    Y_20 = (sqrt5/2)(3 z^2 - 1) is (sqrt5/2)(3 sin^2 theta - 1) in every segment, and Y_00 stays 1."""
+    import math
+    g = ora.Geometry((4, 4, 4), (4, 4), [0.0, 0.9], [0.0, 0.4])
+    phi = np.linspace(0, 2 * math.pi, 13)
+    for tt in (0.0, 0.3, 1.1):
+        q = ora.q_hat(g, phi, tt)
+        assert np.allclose(np.linalg.norm(q, axis=-1), 1.0, atol=1e-15)
+        assert np.allclose(q @ g.vecs["p"], -math.sin(tt / 2), atol=1e-15)
+    c = np.arange(8)
+    s0, s1 = c * 2 * math.pi / 8, (c + 1) * 2 * math.pi / 8            # WAXS: segments over the full circle
+    B0 = ora.basis_matrix(g, 4, s0, s1)
+    assert np.array_equal(B0, ora.basis_matrix(g, 4, s0, s1, two_theta=0.0))
+    tt = 0.8
+    B = ora.basis_matrix(g, 4, s0, s1, two_theta=tt)
+    idx = ora.sh_index(4)
+    i20 = idx.index((2, 0))
+    assert np.allclose(B[0, i20], math.sqrt(5) / 2 * (3 * math.sin(tt / 2) ** 2 - 1), atol=1e-12)
+    assert np.allclose(B[:, 0, :], 1.0, atol=1e-13)
+    assert np.abs(B[1] - B0[1]).max() > 1e-2                          # and it does change the tilted projection
