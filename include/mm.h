@@ -96,6 +96,12 @@ mm_status mm_geometry_get(const mm_geometry *g, int32_t s, double d[3], double j
 mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, int32_t D, const double *seg_start,
                              const double *seg_end, float *h_B);
 
+/* NEXT-4 — as mm_basis_sh_matrix with the full scattering vector of Eq. 1, first line (wide-angle scattering):
+ * q(phi) = cos(2theta/2)(cos(phi) q0 + sin(phi) q90) - sin(2theta/2) p, two_theta in radians (0 = small-angle line).
+ * Y_i(R_s^T q(phi)) is still a trigonometric polynomial of degree <= ell_max in phi: integrated exactly. */
+mm_status mm_basis_sh_matrix_2theta(const mm_geometry *g, int32_t ell_max, double two_theta, int32_t D,
+                                    const double *seg_start, const double *seg_end, float *h_B);
+
 /* NEXT-2 — HOST helper, Eq. 3 for basis sets defined by a grid of orientations: dirs [n_dirs][3] HOST,
  * sample-frame vectors (normalised here); K = n_dirs.
  *   MM_BASIS_NN  nearest-neighbour indicators: B_i(q) = 1 if |q.g_i| is the largest (first on ties), else 0

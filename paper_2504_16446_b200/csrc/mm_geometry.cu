@@ -100,7 +100,7 @@ extern "C" mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometr
     if (!g) { mm_set_error("host allocation failed"); return MM_ERR_ALLOC; }
     for (int i = 0; i < 3; i++) g->shape[i] = desc->volume_shape[i];
     g->J = desc->det_shape[0]; g->Kd = desc->det_shape[1]; g->P = P; g->a = a; g->b = b;
-    memcpy(g->q0, q0, sizeof q0); memcpy(g->q90, q90, sizeof q90);
+    memcpy(g->q0, q0, sizeof q0); memcpy(g->q90, q90, sizeof q90); memcpy(g->p, p, sizeof p);
     g->d_table = nullptr;
     g->host.resize(P);
     g->table.resize(P);
@@ -253,8 +253,8 @@ void real_sh_even(int L, const double n[3], double *Y)
 
 }  // namespace
 
-extern "C" mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, int32_t D, const double *seg_start,
-                                        const double *seg_end, float *h_B)
+static mm_status basis_sh_matrix(const mm_geometry *g, int32_t ell_max, double two_theta, int32_t D, const double *seg_start,
+                                 const double *seg_end, float *h_B)
 {
     if (!g || !seg_start || !seg_end || !h_B) { mm_set_error("mm_basis_sh_matrix: NULL argument"); return MM_ERR_NULL; }
     if (ell_max < 0 || (ell_max & 1) || ell_max > 64 || D < 1) { mm_set_error("ell_max must be even in [0,64], D >= 1"); return MM_ERR_SHAPE; }
@@ -263,12 +263,14 @@ extern "C" mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, i
     // M > 2 ell_max equispaced angles, take its Fourier coefficients, integrate each harmonic in closed form.
     const int M = 2 * ell_max + 2;
     std::vector<double> samp((size_t)M * K), Y(K), ac((size_t)(ell_max + 1) * K), bc((size_t)(ell_max + 1) * K);
+    const double ct = cos(0.5 * two_theta), st = sin(0.5 * two_theta);
     for (int s = 0; s < g->P; s++) {
         const double *R = g->host[s].R;
         for (int t = 0; t < M; t++) {
             const double phi = 2.0 * M_PI * t / M, c = cos(phi), sn = sin(phi);
             double q[3], qs[3];
-            for (int i = 0; i < 3; i++) q[i] = c * g->q0[i] + sn * g->q90[i];        // Eq. 1, small-angle line
+            // Eq. 1: cos(theta)(cos phi q0 + sin phi q90) - sin(theta) p, theta = 2theta/2 (0: the small-angle line)
+            for (int i = 0; i < 3; i++) q[i] = ct * (c * g->q0[i] + sn * g->q90[i]) - st * g->p[i];
             for (int i = 0; i < 3; i++) qs[i] = R[i] * q[0] + R[3 + i] * q[1] + R[6 + i] * q[2];   // R_s^T q
             real_sh_even(ell_max, qs, Y.data());
             for (int i = 0; i < K; i++) samp[(size_t)t * K + i] = Y[i];
@@ -305,6 +307,19 @@ extern "C" mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, i
         }
     }
     return MM_OK;
+}
+
+extern "C" mm_status mm_basis_sh_matrix(const mm_geometry *g, int32_t ell_max, int32_t D, const double *seg_start,
+                                        const double *seg_end, float *h_B)
+{
+    return basis_sh_matrix(g, ell_max, 0.0, D, seg_start, seg_end, h_B);
+}
+
+extern "C" mm_status mm_basis_sh_matrix_2theta(const mm_geometry *g, int32_t ell_max, double two_theta, int32_t D,
+                                               const double *seg_start, const double *seg_end, float *h_B)
+{
+    if (!isfinite(two_theta)) { mm_set_error("mm_basis_sh_matrix_2theta: non-finite 2theta"); return MM_ERR_VALUE; }
+    return basis_sh_matrix(g, ell_max, two_theta, D, seg_start, seg_end, h_B);
 }
 
 // ------------------------------------------------------------------------------------------------

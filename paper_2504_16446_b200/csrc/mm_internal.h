@@ -49,7 +49,7 @@ struct mm_geometry {
     int32_t shape[3];
     int32_t J, Kd, P;
     double a, b;
-    double q0[3], q90[3];
+    double q0[3], q90[3], p[3];
     std::vector<MMProjHost> host;
     std::vector<MMProj> table;
     MMProj *d_table;               // device copy of `table`

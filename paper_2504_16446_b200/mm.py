@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm.so")
 _lib = None
 
-SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_grid_matrix",
+SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
            "mm_axpy_precond", "mm_laplacian", "mm_nesterov_step", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
@@ -51,6 +51,7 @@ def load():
     L.mm_geometry_destroy.argtypes = [vp]
     L.mm_geometry_get.argtypes = [vp, i32, dp, dp, dp, ctypes.POINTER(i32), dp]
     L.mm_basis_sh_matrix.argtypes = [vp, i32, i32, dp, dp, vp]
+    L.mm_basis_sh_matrix_2theta.argtypes = [vp, i32, ctypes.c_double, i32, dp, dp, vp]
     L.mm_basis_grid_matrix.argtypes = [vp, i32, i32, dp, ctypes.c_double, i32, dp, dp, i32, vp]
     L.mm_john_forward.argtypes = [vp, vp, i32, i32, vp, vp]
     L.mm_john_adjoint.argtypes = [vp, vp, i32, i32, vp, vp]
@@ -159,16 +160,21 @@ class Geometry:
         return (self.P,) + self.det + (int(ldk),)
 
 
-def mm_basis_sh_matrix(g: Geometry, ell_max: int, seg_start, seg_end) -> np.ndarray:
-    """host helper: B[P][K][D] float32 (numpy)."""
+def mm_basis_sh_matrix(g: Geometry, ell_max: int, seg_start, seg_end, two_theta: float | None = None) -> np.ndarray:
+    """host helper: B[P][K][D] float32 (numpy); two_theta (radians) selects mm_basis_sh_matrix_2theta."""
     s0 = np.ascontiguousarray(seg_start, dtype=np.float64)
     s1 = np.ascontiguousarray(seg_end, dtype=np.float64)
     D = int(s0.size)
     K = (ell_max + 1) * (ell_max + 2) // 2
     out = np.empty((g.P, K, D), dtype=np.float32)
     dp = ctypes.POINTER(ctypes.c_double)
-    _check(load().mm_basis_sh_matrix(g._h, int(ell_max), D, s0.ctypes.data_as(dp), s1.ctypes.data_as(dp),
-                                     ctypes.c_void_p(out.ctypes.data)), "mm_basis_sh_matrix")
+    if two_theta is None:
+        _check(load().mm_basis_sh_matrix(g._h, int(ell_max), D, s0.ctypes.data_as(dp), s1.ctypes.data_as(dp),
+                                         ctypes.c_void_p(out.ctypes.data)), "mm_basis_sh_matrix")
+    else:
+        _check(load().mm_basis_sh_matrix_2theta(g._h, int(ell_max), float(two_theta), D, s0.ctypes.data_as(dp),
+                                                s1.ctypes.data_as(dp), ctypes.c_void_p(out.ctypes.data)),
+               "mm_basis_sh_matrix_2theta")
     return out
 
 

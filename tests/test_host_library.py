@@ -170,3 +170,18 @@ def test_grid_basis_matrix_rejects_bad_arguments(mm):
         mm.mm_basis_grid_matrix(gm, 7, np.eye(3), s0, s1, sigma=1.0)          # unknown kind
     with pytest.raises(mm.MMError):
         mm.mm_basis_grid_matrix(gm, 1, np.zeros((2, 3)), s0, s1)              # zero direction
+
+
+def test_sh_matrix_full_two_theta_matches_oracle(mm, ora):
+    """NEXT-4: full scattering vector of Eq. 1 (first line) in the SH basis-matrix helper, WAXS-style segments."""
+    r = np.random.default_rng(23)
+    P = 9
+    rot, tilt = r.uniform(0, 2 * math.pi, P), r.uniform(-0.7, 0.7, P)
+    gm = mm.Geometry((5, 6, 7), (6, 5), rot, tilt)
+    go = ora.Geometry((5, 6, 7), (6, 5), rot, tilt)
+    c = np.arange(12)
+    s0, s1 = c * 2 * math.pi / 12, (c + 1) * 2 * math.pi / 12
+    for tt in (0.0, 0.35, 1.2):
+        got = mm.mm_basis_sh_matrix(gm, 6, s0, s1, two_theta=tt)
+        assert np.abs(got - ora.basis_matrix(go, 6, s0, s1, two_theta=tt)).max() < 1e-6
+    assert np.array_equal(mm.mm_basis_sh_matrix(gm, 6, s0, s1, two_theta=0.0), mm.mm_basis_sh_matrix(gm, 6, s0, s1))
