@@ -13,6 +13,7 @@ What is here (numpy, fp64) and what it follows:
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
   basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
   laplacian / laplacian_regulariser / l2_regulariser / nesterov_step   regularisers, momentum   PAPER.md:336-340 (NEXT-3)
+  derived_quantities   mean, second-moment tensor, eigen-decomposition, FA   PAPER.md:198-224, Eq. 10-12 (NEXT-4)
   huber_loss_gradient  Huber-regressor loss and its gradient   PAPER.md:334 (NEXT-4, reading S23)
   sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
 The John transform itself (Joseph's method) is oracle/ora.c, loaded with ctypes.
@@ -474,3 +475,35 @@ def huber_loss_gradient(g: Geometry, B, vol, data, delta, weights=None, form="ga
     rho = np.where(a <= delta, 0.5 * r * r, delta * (a - 0.5 * delta))
     wpsi = w * np.clip(r, -delta, delta)
     return float(np.sum(w * rho)), adjoint(g, B, wpsi, form=form, threads=threads), wpsi
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: derived quantities, PAPER.md:198-224 (Eq. 10-12)
+# ------------------------------------------------------------------------------------------------
+def derived_quantities(coeffs, ell_max, n_theta=None):
+    """For SH coefficients coeffs[..., K] (even l <= ell_max): the definitions written out on a sphere quadrature
+    (Gauss-Legendre in cos(theta) x uniform phi, exact for polynomials of degree <= ell_max + 2):
+        mean  = <f>_q                                   Eq. 10
+        M_ij  = <q_i q_j f(q)>_q                        Eq. 11   (returned as [..., 3, 3])
+        eig   = eigenvalues of M, descending; vec = their eigenvectors (rows, sign arbitrary)
+        FA    = sqrt((l1-l2)^2 + (l2-l3)^2 + (l3-l1)^2) / sqrt(2 (l1^2 + l2^2 + l3^2)),  0 when M = 0     Eq. 12
+    Returns dict(mean, M, eig, vec, fa)."""
+    c = np.asarray(coeffs, dtype=np.float64)
+    nt = n_theta or (ell_max + 4)
+    xs, ws = _leg.leggauss(nt)
+    nphi = 2 * (ell_max + 4)
+    ph = 2.0 * math.pi * np.arange(nphi) / nphi
+    st = np.sqrt(1.0 - xs * xs)
+    q = np.stack([st[:, None] * np.cos(ph)[None, :], st[:, None] * np.sin(ph)[None, :], np.repeat(xs[:, None], nphi, 1)], -1)
+    w = np.repeat((ws / 2.0)[:, None], nphi, 1) / nphi                 # weights of the sphere mean
+    Y = np.stack([real_sh(l, m, q) for (l, m) in sh_index(ell_max)], axis=-1)      # [nt][nphi][K]
+    f = np.tensordot(c, Y, axes=([-1], [-1]))                          # [..., nt, nphi]
+    mean = np.tensordot(f, w, axes=([-2, -1], [0, 1]))
+    M = np.einsum("...tp,tp,tpi,tpj->...ij", f, w, q, q)
+    evals, evecs = np.linalg.eigh(M)
+    eig = evals[..., ::-1]
+    vec = np.swapaxes(evecs, -1, -2)[..., ::-1, :]
+    num = np.sqrt((eig[..., 0] - eig[..., 1]) ** 2 + (eig[..., 1] - eig[..., 2]) ** 2 + (eig[..., 2] - eig[..., 0]) ** 2)
+    den = np.sqrt(2.0 * np.sum(eig * eig, axis=-1))
+    fa = np.where(den > 0, num / np.where(den > 0, den, 1.0), 0.0)
+    return {"mean": mean, "M": M, "eig": eig, "vec": vec, "fa": fa}
