@@ -183,6 +183,17 @@ mm_status mm_residual_loss(const mm_geometry *g, const float *B, const float *vo
 mm_status mm_reciprocal(float *x, int64_t n, float floor, void *stream);
 mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float eta, int64_t n, void *stream);
 
+/* NEXT-4 — derived quantities of a reconstructed SH coefficient volume, per voxel:
+ *   mean [N]               Eq. 10, the isotropic intensity <f> (= coefficient 0 with the 4pi normalisation, S14)
+ *   moments [N][6]         Eq. 11, M_ij = <q_i q_j f>, stored xx, yy, zz, xy, xz, yz
+ *   eigenvalues [N][3]     of M, descending;  eigenvectors [N][3][3] unit row vectors in the same order (sign
+ *                          arbitrary; arbitrary within a degenerate eigenspace)
+ *   fa [N]                 Eq. 12, fractional anisotropy (0 where M = 0)
+ * vol [X][Y][Z][ldk] DEVICE in, real SH of even l in the order of mm_basis_sh_matrix (K = 1 or K >= 6); every
+ * output is DEVICE, N = X*Y*Z, and may be NULL to skip it. */
+mm_status mm_derived_quantities(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *mean, float *moments,
+                                float *eigenvalues, float *eigenvectors, float *fa, void *stream);
+
 /* NEXT-3 — regulariser and optimizer building blocks for a device-resident iteration.
  * mm_laplacian: vol_out[x][i] = sum of the six face neighbours of vol[x][i] - 6 vol[x][i], neighbours outside the
  *   volume counting as 0 (reading S21); vol, vol_out [X][Y][Z][ldk] DEVICE, distinct; pad channels written 0.

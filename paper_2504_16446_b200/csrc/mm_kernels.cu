@@ -615,6 +615,72 @@ __global__ void laplacian_kernel(const float *__restrict__ in, float *__restrict
     Ld<VEC>::st(out + vox * ldk + VEC * e, acc);
 }
 
+// NEXT-4, derived quantities of an SH coefficient volume (Eq. 10-12), one thread per voxel.
+// With 4pi-normalised real harmonics (S14) only l = 0 and l = 2 enter: mean = c_00 and, from <x^2> = 1/3,
+// <x^4> = 1/5, <x^2 y^2> = 1/15 and Y_2,-2..2 = sqrt15 xy, sqrt15 yz, (sqrt5/2)(3z^2-1), sqrt15 xz, (sqrt15/2)(x^2-y^2):
+//   M_xy = c_1/sqrt15, M_yz = c_2/sqrt15, M_xz = c_4/sqrt15,
+//   M_xx = c_0/3 - c_3/(3 sqrt5) + c_5/sqrt15, M_yy = c_0/3 - c_3/(3 sqrt5) - c_5/sqrt15, M_zz = c_0/3 + 2 c_3/(3 sqrt5).
+// Eigenvalues of the symmetric 3x3 by the trigonometric formula, eigenvectors from cross products of the rows of
+// M - lambda I; all in fp64 (a few hundred flops per voxel against 24..192 bytes of traffic).
+__device__ __forceinline__ void eigvec3(const double M[6], double lam, double v[3])
+{
+    // rows of A = M - lam I; the eigenvector is orthogonal to all of them: take the largest cross product
+    const double r0[3] = {M[0] - lam, M[3], M[4]}, r1[3] = {M[3], M[1] - lam, M[5]}, r2[3] = {M[4], M[5], M[2] - lam};
+    double c[3][3] = {{r0[1] * r1[2] - r0[2] * r1[1], r0[2] * r1[0] - r0[0] * r1[2], r0[0] * r1[1] - r0[1] * r1[0]},
+                      {r0[1] * r2[2] - r0[2] * r2[1], r0[2] * r2[0] - r0[0] * r2[2], r0[0] * r2[1] - r0[1] * r2[0]},
+                      {r1[1] * r2[2] - r1[2] * r2[1], r1[2] * r2[0] - r1[0] * r2[2], r1[0] * r2[1] - r1[1] * r2[0]}};
+    int best = 0;
+    double bn = -1.0;
+    for (int i = 0; i < 3; i++) {
+        const double n = c[i][0] * c[i][0] + c[i][1] * c[i][1] + c[i][2] * c[i][2];
+        if (n > bn) { bn = n; best = i; }
+    }
+    if (bn > 0.0) { const double s = rsqrt(bn); v[0] = c[best][0] * s; v[1] = c[best][1] * s; v[2] = c[best][2] * s; }
+    else { v[0] = 1.0; v[1] = 0.0; v[2] = 0.0; }                      // degenerate (isotropic): any unit vector
+}
+
+__global__ void derived_kernel(const float *__restrict__ vol, int ldk, int K, long long nvox, float *__restrict__ mean,
+                               float *__restrict__ moments, float *__restrict__ eig, float *__restrict__ vec, float *__restrict__ fa)
+{
+    const long long vox = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vox >= nvox) return;
+    const float *c = vol + vox * ldk;
+    const double c0 = c[0];
+    double c1 = 0, c2 = 0, c3 = 0, c4 = 0, c5 = 0;
+    if (K >= 6) { c1 = c[1]; c2 = c[2]; c3 = c[3]; c4 = c[4]; c5 = c[5]; }
+    const double i15 = 0.2581988897471611, i35 = 0.14907119849998599;   // 1/sqrt15, 1/(3 sqrt5)
+    double M[6] = {c0 / 3 - c3 * i35 + c5 * i15, c0 / 3 - c3 * i35 - c5 * i15, c0 / 3 + 2 * c3 * i35, c1 * i15, c4 * i15, c2 * i15};
+    const double q = (M[0] + M[1] + M[2]) / 3.0;
+    const double p1 = M[3] * M[3] + M[4] * M[4] + M[5] * M[5];
+    const double d0 = M[0] - q, d1 = M[1] - q, d2 = M[2] - q;
+    const double p = sqrt((d0 * d0 + d1 * d1 + d2 * d2 + 2.0 * p1) / 6.0);
+    double l[3] = {q, q, q};
+    if (p > 0.0) {
+        const double b0 = d0 / p, b1 = d1 / p, b2 = d2 / p, b3 = M[3] / p, b4 = M[4] / p, b5 = M[5] / p;
+        double r = 0.5 * (b0 * (b1 * b2 - b5 * b5) - b3 * (b3 * b2 - b5 * b4) + b4 * (b3 * b5 - b1 * b4));
+        r = fmin(1.0, fmax(-1.0, r));
+        const double phi = acos(r) / 3.0;
+        l[0] = q + 2.0 * p * cos(phi);
+        l[2] = q + 2.0 * p * cos(phi + 2.0943951023931953);
+        l[1] = 3.0 * q - l[0] - l[2];
+    }
+    if (mean) mean[vox] = (float)c0;                                    // Eq. 10: Y_00 = 1
+    if (moments) { for (int i = 0; i < 6; i++) moments[vox * 6 + i] = (float)M[i]; }   // xx, yy, zz, xy, xz, yz  (Eq. 11)
+    if (eig) { eig[vox * 3] = (float)l[0]; eig[vox * 3 + 1] = (float)l[1]; eig[vox * 3 + 2] = (float)l[2]; }
+    if (vec) {
+        for (int i = 0; i < 3; i++) {
+            double v[3];
+            eigvec3(M, l[i], v);
+            vec[vox * 9 + 3 * i] = (float)v[0]; vec[vox * 9 + 3 * i + 1] = (float)v[1]; vec[vox * 9 + 3 * i + 2] = (float)v[2];
+        }
+    }
+    if (fa) {                                                           // Eq. 12
+        const double num = sqrt((l[0] - l[1]) * (l[0] - l[1]) + (l[1] - l[2]) * (l[1] - l[2]) + (l[2] - l[0]) * (l[2] - l[0]));
+        const double den = sqrt(2.0 * (l[0] * l[0] + l[1] * l[1] + l[2] * l[2]));
+        fa[vox] = den > 0.0 ? (float)(num / den) : 0.f;
+    }
+}
+
 // Nesterov momentum (reading S22): v <- m v - eta g;  c <- c + v
 __global__ void nesterov_kernel(float *__restrict__ c, float *__restrict__ v, const float *__restrict__ g, float eta, float m, long long n)
 {
@@ -947,6 +1013,18 @@ extern "C" mm_status mm_laplacian(const mm_geometry *g, const float *vol, int32_
     if (vec) laplacian_kernel<4><<<blocks, 256, 0, (cudaStream_t)stream>>>(vol, vol_out, X, Y, Z, ldk, K);
     else laplacian_kernel<1><<<blocks, 256, 0, (cudaStream_t)stream>>>(vol, vol_out, X, Y, Z, ldk, K);
     return check_launch("laplacian_kernel");
+}
+
+extern "C" mm_status mm_derived_quantities(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *mean, float *moments,
+                                           float *eigenvalues, float *eigenvectors, float *fa, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_derived_quantities");
+    if (st != MM_OK) return st;
+    if (!vol) { mm_set_error("mm_derived_quantities: NULL volume"); return MM_ERR_NULL; }
+    const long long nvox = (long long)g->shape[0] * g->shape[1] * g->shape[2];
+    derived_kernel<<<(unsigned)((nvox + 127) / 128), 128, 0, (cudaStream_t)stream>>>(vol, ldk, K, nvox, mean, moments, eigenvalues,
+                                                                                      eigenvectors, fa);
+    return check_launch("derived_kernel");
 }
 
 extern "C" mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream)

@@ -554,3 +554,45 @@ def test_huber_loss_gradient(ora, mm, weights):
     mm.mm_loss_gradient_huber(gm, dB, dvol, K, dd, dw, 1e30, grad, loss, wr)
     mm.mm_loss_gradient(gm, dB, dvol, K, dd, dw, g2, loss2, wr2)
     assert torch.equal(grad, g2) and torch.equal(wr, wr2) and abs(loss.item() - loss2.item()) <= 1e-12 * loss2.item()
+
+
+@pytest.mark.parametrize("name,shape", [("C3", (14, 12, 16)), ("C1", (9, 11, 7))])
+def test_derived_quantities(ora, mm, name, shape):
+    """NEXT-4 (Eq. 10-12): mean, second-moment tensor, eigen-decomposition and FA of an SH volume.
+    Eigenvectors are unique only up to sign and only where the eigenvalue is isolated: compared as |v.v_ref| there,
+    and checked to be valid (M v = lambda v, unit length) everywhere."""
+    import torch
+    cfg = synth.get_config(name, shape=shape, det=(8, 8), n_rot=2)
+    K, ldk = cfg.K, synth.ldk_for(cfg.K)
+    vol = synth.make_volume(cfg, ldk)
+    vol[..., K:] = 7.0                                                 # pad channels must be ignored
+    vol[0, 0, 0, :K] = 0.0                                             # an empty voxel: M = 0, FA = 0
+    vol[1, 1, 1, :K] = 0.0; vol[1, 1, 1, 0] = 2.0                      # an isotropic voxel: degenerate eigenvalues
+    gm = mm.Geometry(cfg.shape, cfg.det, [0.0], [0.0])
+    mean = torch.empty(cfg.shape, device="cuda"); fa = torch.empty(cfg.shape, device="cuda")
+    mom = torch.empty(cfg.shape + (6,), device="cuda"); eig = torch.empty(cfg.shape + (3,), device="cuda")
+    vec = torch.empty(cfg.shape + (3, 3), device="cuda")
+    mm.mm_derived_quantities(gm, dev(vol), K, mean, mom, eig, vec, fa)
+    d = ora.derived_quantities(vol[..., :K], cfg.ell_max)
+    scale = float(np.abs(d["M"]).max())
+    assert np.abs(mean.cpu().numpy() - d["mean"]).max() <= TOL * np.abs(d["mean"]).max()
+    m = mom.cpu().numpy()
+    Mg = np.stack([np.stack([m[..., 0], m[..., 3], m[..., 4]], -1), np.stack([m[..., 3], m[..., 1], m[..., 5]], -1),
+                   np.stack([m[..., 4], m[..., 5], m[..., 2]], -1)], -2)
+    assert np.abs(Mg - d["M"]).max() <= TOL * scale
+    e = eig.cpu().numpy()
+    assert np.abs(e - d["eig"]).max() <= TOL * scale
+    v = vec.cpu().numpy().astype(np.float64)
+    assert np.abs(np.linalg.norm(v, axis=-1) - 1.0).max() < 1e-5
+    resid = np.einsum("...ij,...kj->...ki", d["M"], v) - d["eig"][..., :, None] * v
+    assert np.abs(resid).max() <= 1e-4 * scale                          # valid eigenvectors everywhere
+    g01, g12 = np.abs(d["eig"][..., 0] - d["eig"][..., 1]), np.abs(d["eig"][..., 1] - d["eig"][..., 2])
+    isolated = [g01 > 1e-2 * scale, np.minimum(g01, g12) > 1e-2 * scale, g12 > 1e-2 * scale]
+    filled = np.abs(d["eig"]).max(axis=-1) > 1e-3 * scale
+    assert filled.any() and isolated[0][filled].mean() > 0.5      # axially symmetric synthetic ODFs: main axis isolated
+    for i in range(3):
+        if isolated[i].any():
+            assert np.abs(np.abs(np.sum(v[..., i, :] * d["vec"][..., i, :], axis=-1))[isolated[i]] - 1.0).max() < 1e-3
+    big = np.abs(d["eig"]).max(axis=-1) > 1e-3 * scale
+    assert np.abs(fa.cpu().numpy() - d["fa"])[big].max() <= 1e-4
+    assert fa[0, 0, 0].item() == 0.0 and abs(fa[1, 1, 1].item()) < 1e-6
