@@ -75,6 +75,19 @@ struct Ld<4> {
     }
 };
 template <>
+struct Ld<8> {                 // 256-bit accesses (sm_100: LDG.E.256 / STG.E.256); p must be 32-byte aligned
+    static __device__ __forceinline__ void ld(const float *p, float (&v)[8])
+    {
+        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p));
+    }
+    static __device__ __forceinline__ void st(float *p, const float (&v)[8])
+    {
+        asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                     ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+    }
+};
+template <>
 struct Ld<1> {
     static __device__ __forceinline__ void ld(const float *p, float (&v)[1]) { v[0] = __ldg(p); }
     static __device__ __forceinline__ void st(float *p, const float (&v)[1]) { *p = v[0]; }
@@ -86,6 +99,19 @@ __device__ __forceinline__ float4 ldg_nc_v4(const float4 *p)
     float4 v;
     asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
+}
+
+// VEC floats (16 or 32 bytes) through the read-only path, in program order like ldg_nc_v4
+template <int VEC>
+__device__ __forceinline__ void ldg_nc_vec(const float *p, float (&v)[VEC])
+{
+    if constexpr (VEC == 4) {
+        asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "l"(p));
+    } else {
+        static_assert(VEC == 8, "vector width");
+        asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p));
+    }
 }
 
 // keep the slabs n in [lo,hi] on which -1 < A + n*s < N can hold (one slab of slack on each side)
@@ -120,7 +146,7 @@ struct __align__(16) SlabTaps {
 // slab nb+q once, parks them in shared memory, and all lanes then stream through G slabs doing nothing but
 // loads and FMAs (v1 spent 21 instructions per LDG.128, profiles/r01_ncu_c5_v1.md).
 template <int VEC, int G, int NQ, int DMAX, int MODE, bool COOP>
-__global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdArgs a)
+__global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_forward_kernel(const FwdArgs a)
 {
     constexpr int RPB = 256 / G;                  // rays per block
     constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
@@ -159,8 +185,11 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
         for (int x = 0; x < VEC; x++) acc[t][x] = 0.f;
 
     if constexpr (COOP) {
-        static_assert(!COOP || VEC == 4, "cooperative march needs float4 lanes");
-        static_assert(G % FWD_U == 0, "a round of G slabs is consumed FWD_U at a time");
+        static_assert(!COOP || VEC == 4 || VEC == 8, "cooperative march needs 16- or 32-byte lanes");
+        // slabs in flight per lane: 32-byte lanes keep a whole round of 8 slabs (32 LDG.256) in flight with 2 blocks
+        // per SM (measured best: 210 ms vs 227 ms for 16-byte lanes, 2 slabs, 4 blocks on config 5)
+        constexpr int U = (VEC == 8) ? 8 : FWD_U;
+        static_assert(G % U == 0, "a round of G slabs is consumed U at a time");
         __shared__ SlabTaps taps[RPB][G];
         int n0 = 0, n1 = -1;
         long long pu0 = 0, pv0 = 0;
@@ -175,9 +204,9 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
             pv0 = (long long)floor(Av * FX_ONE);
         }
         const long long su_fx = pg->su_fx, sv_fx = pg->sv_fx;
-        const int ldk4 = a.ldk >> 2;
-        const int sM4 = (int)(sM >> 2), sU4 = (int)(sU >> 2), sV4 = (int)(sV >> 2);
-        const float4 *vol4 = reinterpret_cast<const float4 *>(a.vol);
+        // tap offsets are counted in lane vectors (VEC floats)
+        const int ldk4 = a.ldk / VEC;
+        const int sM4 = (int)(sM / VEC), sU4 = (int)(sU / VEC), sV4 = (int)(sV / VEC);
         int rounds = (n1 >= n0) ? (n1 - n0 + G) / G : 0;
         rounds = __reduce_max_sync(0xffffffffu, rounds);          // the warp's groups step through rounds together
         for (int rd = 0; rd < rounds; rd++) {
@@ -206,14 +235,14 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
                 taps[r][q] = t;
             }
             __syncwarp();
-            // FWD_U slabs per step: all their loads are issued before the first FMA (slabs past n1 carry
+            // U slabs per step: all their loads are issued before the first FMA (slabs past n1 carry
             // zero weights and offset 0, so the tail needs no special case)
             const int cnt = min(G, n1 - nb + 1);
-            for (int i = 0; i < cnt; i += FWD_U) {
-                int4 o[FWD_U];
-                float4 w[FWD_U];
+            for (int i = 0; i < cnt; i += U) {
+                int4 o[U];
+                float4 w[U];
 #pragma unroll
-                for (int uu = 0; uu < FWD_U; uu++) {
+                for (int uu = 0; uu < U; uu++) {
                     o[uu] = *reinterpret_cast<const int4 *>(&taps[r][i + uu].o00);
                     w[uu] = *reinterpret_cast<const float4 *>(&taps[r][i + uu].w00);
                 }
@@ -222,20 +251,21 @@ __global__ void __launch_bounds__(256, FWD_MINB) john_forward_kernel(const FwdAr
                     // lanes past the last float4 of the voxel re-read its last one (same cache line, result
                     // discarded in the epilogue): no branch in the loop
                     const int e = min(q + G * t, ldk4 - 1);
-                    float4 c[FWD_U][4];
+                    float c[U][4][VEC];
 #pragma unroll
-                    for (int uu = 0; uu < FWD_U; uu++) {
-                        c[uu][0] = ldg_nc_v4(vol4 + (o[uu].x + e)); c[uu][1] = ldg_nc_v4(vol4 + (o[uu].y + e));
-                        c[uu][2] = ldg_nc_v4(vol4 + (o[uu].z + e)); c[uu][3] = ldg_nc_v4(vol4 + (o[uu].w + e));
+                    for (int uu = 0; uu < U; uu++) {
+                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].x + e) * VEC, c[uu][0]);
+                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].y + e) * VEC, c[uu][1]);
+                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].z + e) * VEC, c[uu][2]);
+                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].w + e) * VEC, c[uu][3]);
                     }
 #pragma unroll
-                    for (int uu = 0; uu < FWD_U; uu++) {
+                    for (int uu = 0; uu < U; uu++) {
                         const float ww[4] = {w[uu].x, w[uu].y, w[uu].z, w[uu].w};
 #pragma unroll
-                        for (int p = 0; p < 4; p++) {
-                            acc[t][0] = fmaf(ww[p], c[uu][p].x, acc[t][0]); acc[t][1] = fmaf(ww[p], c[uu][p].y, acc[t][1]);
-                            acc[t][2] = fmaf(ww[p], c[uu][p].z, acc[t][2]); acc[t][3] = fmaf(ww[p], c[uu][p].w, acc[t][3]);
-                        }
+                        for (int p = 0; p < 4; p++)
+#pragma unroll
+                            for (int x = 0; x < VEC; x++) acc[t][x] = fmaf(ww[p], c[uu][p][x], acc[t][x]);
                     }
                 }
             }
@@ -733,9 +763,9 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
     constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
     constexpr int TJ = RPB / TK;
     const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
-    if constexpr (VEC == 4 && G >= FWD_U) {
-        // cooperative march: tap offsets are 32-bit float4 indices
-        if ((long long)a.X * a.Y * a.Z * (a.ldk / 4) < (1LL << 31)) {
+    if constexpr ((VEC == 4 && G >= FWD_U) || (VEC == 8 && G % 8 == 0)) {
+        // cooperative march: tap offsets are 32-bit lane-vector indices
+        if ((long long)a.X * a.Y * a.Z * (a.ldk / VEC) < (1LL << 31)) {
             john_forward_kernel<VEC, G, NQ, DMAX, MODE, true><<<(unsigned)tiles, 256, 0, st>>>(a);
             return;
         }
@@ -746,6 +776,13 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
 template <int DMAX, int MODE>
 mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
 {
+    // 32-byte lanes (LDG.E.256): 8 lanes cover up to 64 channels, 16 lanes up to 128
+    if (vec && a.ldk % 8 == 0 && a.ldk >= 40 && a.ldk <= 128 && (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0 &&
+        (reinterpret_cast<uintptr_t>(a.proj) & 31u) == 0) {
+        if (a.ldk <= 64) launch_fwd<8, 8, 1, DMAX, MODE>(a, st);
+        else launch_fwd<8, 16, 1, DMAX, MODE>(a, st);
+        return check_launch("john_forward_kernel");
+    }
     if (vec) {
         const int lpv = a.ldk / 4;
         if (lpv <= 1) launch_fwd<4, 1, 1, DMAX, MODE>(a, st);
