@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_f
         static_assert(!COOP || VEC == 4 || VEC == 8, "cooperative march needs 16- or 32-byte lanes");
         // slabs in flight per lane: 32-byte lanes keep a whole round of 8 slabs (32 LDG.256) in flight with 2 blocks
         // per SM (measured best: 210 ms vs 227 ms for 16-byte lanes, 2 slabs, 4 blocks on config 5)
-        constexpr int U = (VEC == 8) ? 8 : FWD_U;
+        constexpr int U = (VEC == 8) ? (G < 8 ? G : 8) : FWD_U;
         static_assert(G % U == 0, "a round of G slabs is consumed U at a time");
         __shared__ SlabTaps taps[RPB][G];
         int n0 = 0, n1 = -1;
@@ -763,7 +763,7 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
     constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
     constexpr int TJ = RPB / TK;
     const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
-    if constexpr ((VEC == 4 && G >= FWD_U) || (VEC == 8 && G % 8 == 0)) {
+    if constexpr ((VEC == 4 && G >= FWD_U) || (VEC == 8 && G >= 4)) {
         // cooperative march: tap offsets are 32-bit lane-vector indices
         if ((long long)a.X * a.Y * a.Z * (a.ldk / VEC) < (1LL << 31)) {
             john_forward_kernel<VEC, G, NQ, DMAX, MODE, true><<<(unsigned)tiles, 256, 0, st>>>(a);
@@ -776,10 +776,11 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
 template <int DMAX, int MODE>
 mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
 {
-    // 32-byte lanes (LDG.E.256): 8 lanes cover up to 64 channels, 16 lanes up to 128
-    if (vec && a.ldk % 8 == 0 && a.ldk >= 40 && a.ldk <= 128 && (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0 &&
+    // 32-byte lanes (LDG.E.256): 4 lanes cover up to 32 channels, 8 lanes up to 64, 16 lanes up to 128
+    if (vec && a.ldk % 8 == 0 && a.ldk >= 24 && a.ldk <= 128 && (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0 &&
         (reinterpret_cast<uintptr_t>(a.proj) & 31u) == 0) {
-        if (a.ldk <= 64) launch_fwd<8, 8, 1, DMAX, MODE>(a, st);
+        if (a.ldk <= 32) launch_fwd<8, 4, 1, DMAX, MODE>(a, st);
+        else if (a.ldk <= 64) launch_fwd<8, 8, 1, DMAX, MODE>(a, st);
         else launch_fwd<8, 16, 1, DMAX, MODE>(a, st);
         return check_launch("john_forward_kernel");
     }

@@ -59,8 +59,8 @@ def n_coeffs(ell_max: int) -> int:
 
 
 def ldk_for(K: int) -> int:
-    """channel stride (floats) used by the fast path: next multiple of 4."""
-    return (K + 3) // 4 * 4
+    """channel stride (floats) used by the fast paths: next multiple of 4, or of 8 (32-byte lanes) from K > 20."""
+    return (K + 7) // 8 * 8 if K > 20 else (K + 3) // 4 * 4
 
 
 CONFIGS = {
