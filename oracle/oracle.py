@@ -13,6 +13,7 @@ What is here (numpy, fp64) and what it follows:
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
   basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
   laplacian / laplacian_regulariser / l2_regulariser / nesterov_step   regularisers, momentum   PAPER.md:336-340 (NEXT-3)
+  l1_regulariser / huber_norm_regulariser / total_variation_regulariser   PAPER.md:336-338 (NEXT-3, reading S24)
   derived_quantities   mean, second-moment tensor, eigen-decomposition, FA   PAPER.md:198-224, Eq. 10-12 (NEXT-4)
   huber_loss_gradient  Huber-regressor loss and its gradient   PAPER.md:334 (NEXT-4, reading S23)
   sirt_preconditioners / sirt_step   SIRT/MITRA as preconditioned weighted least squares  PAPER.md:258-262, reading S19
@@ -507,3 +508,46 @@ def derived_quantities(coeffs, ell_max, n_theta=None):
     den = np.sqrt(2.0 * np.sum(eig * eig, axis=-1))
     fa = np.where(den > 0, num / np.where(den > 0, den, 1.0), 0.0)
     return {"mean": mean, "M": M, "eig": eig, "vec": vec, "fa": fa}
+
+
+def _huber(t, delta):
+    """Huber function of PAPER.md:336-338 ("acts as an L1 norm for large values and an L2 norm for small values"),
+    reading S24: h(t) = t^2 / (2 delta) for |t| <= delta, |t| - delta/2 beyond (slope 1 far out, C^1)."""
+    a = np.abs(t)
+    return np.where(a <= delta, t * t / (2.0 * delta), a - 0.5 * delta)
+
+
+def l1_regulariser(vol):
+    """(R, grad) of L1Norm: R = sum |c|, grad = sign(c) (0 at 0)."""
+    v = np.asarray(vol, dtype=np.float64)
+    return float(np.sum(np.abs(v))), np.sign(v)
+
+
+def huber_norm_regulariser(vol, delta):
+    """(R, grad) of HuberNorm: R = sum h(c), grad = clip(c / delta, -1, 1)."""
+    v = np.asarray(vol, dtype=np.float64)
+    return float(np.sum(_huber(v, delta))), np.clip(v / delta, -1.0, 1.0)
+
+
+def total_variation_regulariser(vol, delta):
+    """(R, grad) of TotalVariation ("the Huber norm of the spatial gradient for each basis-set mode"),
+    reading S24: forward differences d_a c[x] = c[x + e_a] - c[x] (0 across the last face), per voxel and channel
+    n = sqrt(sum_a (d_a c)^2), R = sum h(n); grad = D^T ( h'(n) d c / n ) with h'(n)/n = 1 / max(n, delta)."""
+    v = np.asarray(vol, dtype=np.float64)
+    d = np.zeros((3,) + v.shape)
+    for ax in range(3):
+        lo = [slice(None)] * 4
+        hi = [slice(None)] * 4
+        lo[ax], hi[ax] = slice(0, -1), slice(1, None)
+        d[(ax,) + tuple(lo)] = v[tuple(hi)] - v[tuple(lo)]
+    n = np.sqrt(np.sum(d * d, axis=0))
+    R = float(np.sum(_huber(n, delta)))
+    p = d / np.maximum(n, delta)
+    g = np.zeros_like(v)
+    for ax in range(3):
+        lo = [slice(None)] * 4
+        hi = [slice(None)] * 4
+        lo[ax], hi[ax] = slice(0, -1), slice(1, None)
+        g[tuple(lo)] -= p[(ax,) + tuple(lo)]
+        g[tuple(hi)] += p[(ax,) + tuple(lo)]
+    return R, g

@@ -54,3 +54,31 @@ def test_nesterov_reduces_to_plain_descent_and_accelerates(ora):
             x, vel = ora.nesterov_step(x, vel, A @ (x + m * vel), eta=0.009, momentum=m)
         return 0.5 * x @ A @ x
     assert run(0.9) < 1e-2 * run(0.0)
+
+
+def test_l1_huber_norm_total_variation(ora):
+    """PAPER.md:336-338, reading S24.  Closed forms: a linear ramp c = a x + b y has |grad c| = sqrt(a^2+b^2) at every
+    voxel that has both forward neighbours; HuberNorm tends to L1 - delta/2 per element for delta -> 0 and to
+    L2/(delta) for large delta; gradients by finite differences (the Huberised terms are C^1)."""
+    r = np.random.default_rng(4)
+    c = r.standard_normal((6, 5, 7, 2))
+    R1, g1 = ora.l1_regulariser(c)
+    assert abs(R1 - np.abs(c).sum()) < 1e-12 and np.array_equal(g1, np.sign(c))
+    Rh, gh = ora.huber_norm_regulariser(c, 1e-9)
+    assert abs(Rh - (R1 - 0.5e-9 * c.size)) < 1e-9 and np.array_equal(gh, np.sign(c))
+    Rh, gh = ora.huber_norm_regulariser(c, 1e3)
+    assert abs(Rh - 0.5 * np.sum(c * c) / 1e3) < 1e-12 and np.allclose(gh, c / 1e3)
+    X, Y, Z = 6, 5, 4
+    x, y, z = np.meshgrid(np.arange(X), np.arange(Y), np.arange(Z), indexing="ij")
+    ramp = (3.0 * x + 4.0 * y)[..., None].astype(float)
+    Rt, gt = ora.total_variation_regulariser(ramp, 0.1)
+    full = (X - 1) * (Y - 1) * Z * (5.0 - 0.05)                       # both differences present: |grad| = 5
+    edge_x = (Y - 1) * Z * (4.0 - 0.05)                               # last x plane: only d_y = 4
+    edge_y = (X - 1) * Z * (3.0 - 0.05)                               # last y row: only d_x = 3
+    assert abs(Rt - (full + edge_x + edge_y)) < 1e-10                 # the corner column has no difference at all
+    assert abs(gt[2, 2, 1, 0]) < 1e-12                                # interior of a linear ramp: zero TV gradient
+    for reg in (lambda v: ora.huber_norm_regulariser(v, 0.3), lambda v: ora.total_variation_regulariser(v, 0.3)):
+        d = r.standard_normal(c.shape)
+        h = 1e-6
+        fd = (reg(c + h * d)[0] - reg(c - h * d)[0]) / (2 * h)
+        assert abs(fd - np.sum(reg(c)[1] * d)) < 1e-5 * max(1.0, abs(fd))
