@@ -202,6 +202,19 @@ mm_status mm_derived_quantities(const mm_geometry *g, const float *vol, int32_t 
  * mm_nesterov_step: v <- momentum v - eta grad;  c <- c + v  (GradientDescent with Nesterov momentum; the
  *   caller evaluates grad at c + momentum v, reading S22); n floats each, DEVICE. */
 mm_status mm_laplacian(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *vol_out, void *stream);
+
+/* The other regularisers of P:336-338 (reading S24; h(t) = t^2/(2 delta) for |t| <= delta, |t| - delta/2 beyond):
+ *   MM_REG_L1     L1Norm         R = sum |c|,                  grad = sign(c)               (delta ignored)
+ *   MM_REG_HUBER  HuberNorm      R = sum h(c),                 grad = clip(c/delta, -1, 1)
+ *   MM_REG_TV     TotalVariation R = sum_x,i h(|D c_i(x)|),    grad = D^T (D c_i / max(|D c_i|, delta)),
+ *                 D = forward differences along x, y, z (0 across the last face), per channel i.
+ * vol [X][Y][Z][ldk] DEVICE in; grad_out same shape, DEVICE out (overwritten, pad channels 0), distinct from vol;
+ * value: DEVICE double, overwritten with R, or NULL. */
+#define MM_REG_L1 1
+#define MM_REG_HUBER 2
+#define MM_REG_TV 3
+mm_status mm_regulariser(const mm_geometry *g, int32_t kind, const float *vol, int32_t K, int32_t ldk, float delta,
+                         float *grad_out, double *value, void *stream);
 mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream);
 
 /* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */

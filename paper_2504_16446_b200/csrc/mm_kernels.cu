@@ -711,6 +711,67 @@ __global__ void derived_kernel(const float *__restrict__ vol, int ldk, int K, lo
     }
 }
 
+// NEXT-3 regularisers (reading S24), one thread per (voxel, channel): value (fp64, one atomic per
+// block) and gradient.  kind 1: L1Norm, 2: HuberNorm, 3: TotalVariation (Huber norm of the forward-difference
+// gradient per channel).  h(t) = t^2/(2 delta) for |t| <= delta, |t| - delta/2 beyond.
+__device__ __forceinline__ float reg_huber(float t, float delta)
+{
+    const float a = fabsf(t);
+    return a <= delta ? t * t / (2.f * delta) : a - 0.5f * delta;
+}
+// forward differences of channel i at voxel (x,y,z) (0 across the last face) and their Euclidean norm
+__device__ __forceinline__ float tv_diffs(const float *__restrict__ v, int x, int y, int z, int X, int Y, int Z, long long sX,
+                                          long long sY, long long sZ, float (&d)[3])
+{
+    const float *p = v + x * sX + y * sY + z * sZ;
+    const float c = __ldg(p);
+    d[0] = x + 1 < X ? __ldg(p + sX) - c : 0.f;
+    d[1] = y + 1 < Y ? __ldg(p + sY) - c : 0.f;
+    d[2] = z + 1 < Z ? __ldg(p + sZ) - c : 0.f;
+    return sqrtf(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+}
+__global__ void __launch_bounds__(256) regulariser_kernel(const float *__restrict__ vol, float *__restrict__ grad, double *__restrict__ value,
+                                                          int kind, float delta, int X, int Y, int Z, int ldk, int K)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)X * Y * Z * ldk;
+    double r = 0.0;
+    if (idx < total) {
+        const int i = (int)(idx % ldk);
+        const long long vox = idx / ldk;
+        float g = 0.f;
+        if (i < K) {
+            const float c = __ldg(vol + idx);
+            if (kind == 1) { r = fabsf(c); g = c > 0.f ? 1.f : (c < 0.f ? -1.f : 0.f); }
+            else if (kind == 2) { r = reg_huber(c, delta); g = fminf(1.f, fmaxf(-1.f, c / delta)); }
+            else {
+                const int z = (int)(vox % Z), y = (int)((vox / Z) % Y), x = (int)(vox / ((long long)Z * Y));
+                const long long sZ = ldk, sY = (long long)Z * ldk, sX = (long long)Y * Z * ldk;
+                const float *v = vol + i;
+                float d[3], dn[3];
+                const float n = tv_diffs(v, x, y, z, X, Y, Z, sX, sY, sZ, d);
+                r = reg_huber(n, delta);
+                g = -(d[0] + d[1] + d[2]) / fmaxf(n, delta);                         // - sum_a p_a(x)
+                if (x > 0) { const float m = tv_diffs(v, x - 1, y, z, X, Y, Z, sX, sY, sZ, dn); g += dn[0] / fmaxf(m, delta); }
+                if (y > 0) { const float m = tv_diffs(v, x, y - 1, z, X, Y, Z, sX, sY, sZ, dn); g += dn[1] / fmaxf(m, delta); }
+                if (z > 0) { const float m = tv_diffs(v, x, y, z - 1, X, Y, Z, sX, sY, sZ, dn); g += dn[2] / fmaxf(m, delta); }
+            }
+        }
+        grad[idx] = g;
+    }
+    if (value) {
+        __shared__ double red[8];
+        r = warp_sum(r);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = r;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < 8; w++) tot += red[w];
+            if (tot != 0.0) atomicAdd(value, tot);
+        }
+    }
+}
+
 // Nesterov momentum (reading S22): v <- m v - eta g;  c <- c + v
 __global__ void nesterov_kernel(float *__restrict__ c, float *__restrict__ v, const float *__restrict__ g, float eta, float m, long long n)
 {
@@ -1063,6 +1124,26 @@ extern "C" mm_status mm_derived_quantities(const mm_geometry *g, const float *vo
     derived_kernel<<<(unsigned)((nvox + 127) / 128), 128, 0, (cudaStream_t)stream>>>(vol, ldk, K, nvox, mean, moments, eigenvalues,
                                                                                       eigenvectors, fa);
     return check_launch("derived_kernel");
+}
+
+extern "C" mm_status mm_regulariser(const mm_geometry *g, int32_t kind, const float *vol, int32_t K, int32_t ldk, float delta,
+                                    float *grad_out, double *value, void *stream)
+{
+    mm_status st = check_common(g, K, ldk, "mm_regulariser");
+    if (st != MM_OK) return st;
+    if (!vol || !grad_out) { mm_set_error("mm_regulariser: NULL buffer"); return MM_ERR_NULL; }
+    if (vol == grad_out) { mm_set_error("mm_regulariser: in and out must differ"); return MM_ERR_VALUE; }
+    if (kind != MM_REG_L1 && kind != MM_REG_HUBER && kind != MM_REG_TV) { mm_set_error("mm_regulariser: unknown kind"); return MM_ERR_VALUE; }
+    if (kind != MM_REG_L1 && !(delta > 0.f)) { mm_set_error("mm_regulariser: delta must be positive"); return MM_ERR_VALUE; }
+    cudaStream_t cs = (cudaStream_t)stream;
+    if (value && cudaMemsetAsync(value, 0, sizeof(double), cs) != cudaSuccess) {
+        mm_set_error(std::string("cudaMemsetAsync(value): ") + cudaGetErrorString(cudaGetLastError()));
+        return MM_ERR_CUDA;
+    }
+    const int X = g->shape[0], Y = g->shape[1], Z = g->shape[2];
+    const long long total = (long long)X * Y * Z * ldk;
+    regulariser_kernel<<<(unsigned)((total + 255) / 256), 256, 0, cs>>>(vol, grad_out, value, kind, delta, X, Y, Z, ldk, K);
+    return check_launch("regulariser_kernel");
 }
 
 extern "C" mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream)

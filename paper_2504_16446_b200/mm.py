@@ -19,7 +19,7 @@ _lib = None
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
-           "mm_axpy_precond", "mm_laplacian", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
+           "mm_axpy_precond", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -67,6 +67,7 @@ def load():
     L.mm_loss_gradient_huber.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, ctypes.c_float, vp, vp, vp, vp]
     L.mm_reciprocal.argtypes = [vp, i64, ctypes.c_float, vp]
     L.mm_laplacian.argtypes = [vp, vp, i32, i32, vp, vp]
+    L.mm_regulariser.argtypes = [vp, i32, vp, i32, i32, ctypes.c_float, vp, vp, vp]
     L.mm_derived_quantities.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
     L.mm_nesterov_step.argtypes = [vp, vp, vp, ctypes.c_float, ctypes.c_float, i64, vp]
     L.mm_axpy_precond.argtypes = [vp, vp, vp, ctypes.c_float, i64, vp]
@@ -313,6 +314,19 @@ def mm_derived_quantities(g: Geometry, vol, K: int, mean=None, moments=None, eig
                                         opt(moments, n + (6,), "moments"), opt(eigenvalues, n + (3,), "eigenvalues"),
                                         opt(eigenvectors, n + (3, 3), "eigenvectors"), opt(fa, n, "fa"), _stream(stream)),
            "mm_derived_quantities")
+
+
+MM_REG_L1, MM_REG_HUBER, MM_REG_TV = 1, 2, 3
+
+
+def mm_regulariser(g: Geometry, kind: int, vol, K: int, delta: float, grad_out, value=None, stream=None):
+    """value: CUDA float64 tensor with one element (overwritten) or None."""
+    import torch
+    ldk = vol.shape[-1]
+    v = ctypes.c_void_p(None) if value is None else _dev(value, (1,), "value", torch.float64)
+    _check(load().mm_regulariser(g._h, int(kind), _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, float(delta),
+                                 _dev(grad_out, g.vol_shape(ldk), "grad_out"), v, _stream(stream)), "mm_regulariser")
+    return grad_out
 
 
 def mm_nesterov_step(c, v, grad, eta: float, momentum: float, stream=None):

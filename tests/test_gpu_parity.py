@@ -596,3 +596,21 @@ def test_derived_quantities(ora, mm, name, shape):
     big = np.abs(d["eig"]).max(axis=-1) > 1e-3 * scale
     assert np.abs(fa.cpu().numpy() - d["fa"])[big].max() <= 1e-4
     assert fa[0, 0, 0].item() == 0.0 and abs(fa[1, 1, 1].item()) < 1e-6
+
+
+@pytest.mark.parametrize("K,ldk,shape", [(6, 8, (13, 11, 15)), (5, 5, (7, 1, 9)), (45, 48, (10, 12, 8))])
+def test_l1_huber_tv_regularisers(ora, mm, K, ldk, shape):
+    """NEXT-3 (reading S24): value and gradient of L1Norm, HuberNorm and TotalVariation."""
+    import torch
+    gm = mm.Geometry(shape, (4, 4), [0.0], [0.0])
+    v = np.random.default_rng(K).standard_normal(shape + (ldk,)).astype(np.float32)
+    dv = dev(v)
+    for kind, fn in [(mm.MM_REG_L1, lambda c: ora.l1_regulariser(c)), (mm.MM_REG_HUBER, lambda c: ora.huber_norm_regulariser(c, 0.4)),
+                     (mm.MM_REG_TV, lambda c: ora.total_variation_regulariser(c, 0.4))]:
+        grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+        val = torch.full((1,), float("nan"), device="cuda", dtype=torch.float64)
+        mm.mm_regulariser(gm, kind, dv, K, 0.4, grad, val)
+        R, g_o = fn(v[..., :K])
+        got = grad.cpu().numpy()
+        assert abs(val.item() - R) <= 1e-5 * R
+        assert np.abs(got[..., :K] - g_o).max() <= 2e-5 * max(1.0, np.abs(g_o).max()) and np.all(got[..., K:] == 0.0)
