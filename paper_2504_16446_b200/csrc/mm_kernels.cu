@@ -190,7 +190,11 @@ __global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_f
         // per SM (measured best: 210 ms vs 227 ms for 16-byte lanes, 2 slabs, 4 blocks on config 5)
         constexpr int U = (VEC == 8) ? (G < 8 ? G : 8) : FWD_U;
         static_assert(G % U == 0, "a round of G slabs is consumed U at a time");
-        __shared__ SlabTaps taps[RPB][G];
+        // offsets and weights in separate arrays, each ray's row padded by one entry: the rays of a warp then sit in
+        // different banks (the [RPB][G] array of 32-byte structs put them all on the same four banks: 9.5 shared
+        // wavefronts per warp and slab in profiles/r01_ncu_c5_v4.md, against 3 without conflicts)
+        __shared__ int4 tap_o[RPB][G + 1];
+        __shared__ float4 tap_w[RPB][G + 1];
         int n0 = 0, n1 = -1;
         long long pu0 = 0, pv0 = 0;
         if (ray_ok) {
@@ -232,7 +236,8 @@ __global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_f
                     t.w01 = (u0 && v1) ? (1.f - fu) * fv : 0.f;
                     t.w11 = (u1 && v1) ? fu * fv : 0.f;
                 }
-                taps[r][q] = t;
+                tap_o[r][q] = make_int4(t.o00, t.o10, t.o01, t.o11);
+                tap_w[r][q] = make_float4(t.w00, t.w10, t.w01, t.w11);
             }
             __syncwarp();
             // U slabs per step: all their loads are issued before the first FMA (slabs past n1 carry
@@ -243,8 +248,8 @@ __global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_f
                 float4 w[U];
 #pragma unroll
                 for (int uu = 0; uu < U; uu++) {
-                    o[uu] = *reinterpret_cast<const int4 *>(&taps[r][i + uu].o00);
-                    w[uu] = *reinterpret_cast<const float4 *>(&taps[r][i + uu].w00);
+                    o[uu] = tap_o[r][i + uu];
+                    w[uu] = tap_w[r][i + uu];
                 }
 #pragma unroll
                 for (int t = 0; t < NQ; t++) {
