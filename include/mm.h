@@ -220,9 +220,13 @@ mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, flo
 /* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */
 mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream);
 
-/* End-to-end convenience with HOST buffers (what a caller without device memory uses): allocates device
- * buffers, copies B, vol, data, weights host->device, runs mm_loss_gradient, copies grad and loss back,
- * frees, and synchronises.  All pointers HOST; h_weights may be NULL; h_loss is one double. */
+/* End-to-end convenience with HOST buffers (what a caller without device memory uses): copies B, vol, data,
+ * weights host->device, runs mm_loss_gradient, copies grad and loss back, and synchronises.  All pointers
+ * HOST (pinned memory makes the copies asynchronous DMA); h_weights may be NULL; h_loss is one double.
+ * The device workspace (one arena of 2 volumes + 2-3 sinograms + B, and one stream) is owned by the library,
+ * grows on demand, is reused by later calls and is freed by mm_host_workspace_release(); calls are serialised
+ * inside the library.  MM_ERR_ALLOC if the arena cannot be allocated (nothing is left allocated then). */
+mm_status mm_host_workspace_release(void);
 mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K,
                                 int32_t ldk, int32_t D, const float *h_data, const float *h_weights,
                                 float *h_grad, double *h_loss);

@@ -415,8 +415,8 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MINB) adjoint_tc_kernel(const A
         }
     } else {
         // ---------------- gather warps ----------------
-        const long long nvox = (long long)a.X * a.Y * a.Z;
-        const long long vox = (long long)blockIdx.x * TC_M + tid;
+        const long long nvox = a.vox_end;
+        const long long vox = a.vox_begin + (long long)blockIdx.x * TC_M + tid;
         const bool ok = vox < nvox;
         const long long vv = ok ? vox : nvox - 1;
         const int z = (int)(vv % a.Z), y = (int)((vv / a.Z) % a.Y), x = (int)(vv / ((long long)a.Z * a.Y));
@@ -523,7 +523,8 @@ cudaError_t launch_tc(const AdjArgs &a, cudaStream_t st)
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const long long nvox = (long long)a.X * a.Y * a.Z;
+    const long long nvox = a.vox_end - a.vox_begin;
+    if (nvox <= 0) return cudaSuccess;
     adjoint_tc_kernel<D, NPAD><<<(unsigned)((nvox + TC_M - 1) / TC_M), TC_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }

@@ -67,6 +67,7 @@ struct AdjArgs {
     int K, ldk, D;
     int X, Y, Z, J, Kd, P;
     int vec_ok;               // fused: D % 4 == 0 and src 16-byte aligned
+    long long vox_begin, vox_end;   // fused kernels: voxels [vox_begin, vox_end) of the launch (whole volume by default)
     int bilinear;             // 0: exact transpose of the Joseph forward (S9); 1: the paper's bilinear back-projection
 };
 

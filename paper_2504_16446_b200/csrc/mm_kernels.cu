@@ -14,6 +14,7 @@
 #include <stdlib.h>
 
 #include <atomic>
+#include <mutex>
 #include <string>
 
 #include "mm_internal.h"
@@ -38,6 +39,15 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
 #endif
 #ifndef FWD_U
 #define FWD_U 2                         // slabs in flight per lane in the cooperative forward march
+#endif
+#ifndef FWD_U8
+#define FWD_U8 8                        // same, for 32-byte lanes: a whole round of 8 slabs
+#endif
+#ifndef FWD_MINB8
+#define FWD_MINB8 2                     // resident blocks per SM asked of the compiler for 32-byte lanes
+#endif
+#ifndef FWD_TK
+#define FWD_TK 4                        // rays along k in the tile of a 32-ray block
 #endif
 #define FX_ONE 4294967296.0            // 2^32
 #define FX_INV 2.3283064365386963e-10f // 2^-32
@@ -146,10 +156,10 @@ struct __align__(16) SlabTaps {
 // slab nb+q once, parks them in shared memory, and all lanes then stream through G slabs doing nothing but
 // loads and FMAs (v1 spent 21 instructions per LDG.128, profiles/r01_ncu_c5_v1.md).
 template <int VEC, int G, int NQ, int DMAX, int MODE, bool COOP>
-__global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_forward_kernel(const FwdArgs a)
+__global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MINB8 : FWD_MINB) john_forward_kernel(const FwdArgs a)
 {
     constexpr int RPB = 256 / G;                  // rays per block
-    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
+    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 32 ? FWD_TK : (RPB >= 4 ? 4 : RPB));
     constexpr int TJ = RPB / TK;
     const int tid = threadIdx.x;
     const int q = tid % G;                        // lane within the ray's group
@@ -188,7 +198,7 @@ __global__ void __launch_bounds__(256, (COOP && VEC == 8) ? 2 : FWD_MINB) john_f
         static_assert(!COOP || VEC == 4 || VEC == 8, "cooperative march needs 16- or 32-byte lanes");
         // slabs in flight per lane: 32-byte lanes keep a whole round of 8 slabs (32 LDG.256) in flight with 2 blocks
         // per SM (measured best: 210 ms vs 227 ms for 16-byte lanes, 2 slabs, 4 blocks on config 5)
-        constexpr int U = (VEC == 8) ? (G < 8 ? G : 8) : FWD_U;
+        constexpr int U = (VEC == 8) ? (G < FWD_U8 ? G : FWD_U8) : (NQ >= 3 ? (G < 4 ? G : 4) : FWD_U);
         static_assert(G % U == 0, "a round of G slabs is consumed U at a time");
         // offsets and weights in separate arrays, each ray's row padded by one entry: the rays of a warp then sit in
         // different banks (the [RPB][G] array of 32-byte structs put them all on the same four banks: 9.5 shared
@@ -482,8 +492,8 @@ __global__ void __launch_bounds__(128) adjoint_fused_kernel(const AdjArgs a)
     __shared__ AdjProjS sp[ADJ_PCH];
     __shared__ __align__(16) float sB[ADJ_PCH][KMAX * DMAX];
     const int tid = threadIdx.x;
-    const long long vox = (long long)blockIdx.x * 128 + tid;
-    const long long nvox = (long long)a.X * a.Y * a.Z;
+    const long long vox = a.vox_begin + (long long)blockIdx.x * 128 + tid;
+    const long long nvox = a.vox_end;
     const bool ok = vox < nvox;
     const long long vv = ok ? vox : nvox - 1;
     const int z = (int)(vv % a.Z), y = (int)((vv / a.Z) % a.Y), x = (int)(vv / ((long long)a.Z * a.Y));
@@ -826,7 +836,7 @@ template <int VEC, int G, int NQ, int DMAX, int MODE>
 void launch_fwd(const FwdArgs &a, cudaStream_t st)
 {
     constexpr int RPB = 256 / G;
-    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 4 ? 4 : RPB);
+    constexpr int TK = (RPB >= 64) ? 8 : (RPB >= 32 ? FWD_TK : (RPB >= 4 ? 4 : RPB));
     constexpr int TJ = RPB / TK;
     const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
     if constexpr ((VEC == 4 && G >= FWD_U) || (VEC == 8 && G >= 4)) {
@@ -842,6 +852,10 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
 template <int DMAX, int MODE>
 mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
 {
+    // 48 floats per voxel (K = 45, configs 3 and 5) = 12 float4 = 4 lanes x 3: every lane's load is used.  The
+    // 8 x 32-byte layout below would idle 2 lanes in 8, and the register write-back of a load costs the same
+    // 8 wavefronts whether or not its lanes carry new data (profiles/r01_ncu_c5_v5.md): 198 -> 191 ms on config 5.
+    if (vec && a.ldk == 48) { launch_fwd<4, 4, 3, DMAX, MODE>(a, st); return check_launch("john_forward_kernel"); }
     // 32-byte lanes (LDG.E.256): 4 lanes cover up to 32 channels, 8 lanes up to 64, 16 lanes up to 128
     if (vec && a.ldk % 8 == 0 && a.ldk >= 24 && a.ldk <= 128 && (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0 &&
         (reinterpret_cast<uintptr_t>(a.proj) & 31u) == 0) {
@@ -888,6 +902,7 @@ void fill_adj(AdjArgs &a, const mm_geometry *g, const float *src, const float *B
     a.tab = g->d_table; a.src = src; a.B = B; a.out = out; a.K = K; a.ldk = ldk; a.D = D;
     a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
     a.vec_ok = 0; a.bilinear = 0;
+    a.vox_begin = 0; a.vox_end = (long long)a.X * a.Y * a.Z;
 }
 
 template <int VEC, int G, int NQ>
@@ -901,7 +916,8 @@ void launch_adj(const AdjArgs &a, cudaStream_t st)
 template <int KMAX>
 mm_status launch_adj_fused(const AdjArgs &a, cudaStream_t st)
 {
-    const long long nvox = (long long)a.X * a.Y * a.Z;
+    const long long nvox = a.vox_end - a.vox_begin;
+    if (nvox <= 0) return MM_OK;
     dim3 grid((unsigned)((nvox + 127) / 128), (unsigned)((a.ldk + KMAX - 1) / KMAX));
     // chunks past K only need to zero the pad channels; they still run the (cheap for them) common path
     if (a.D <= 8) adjoint_fused_kernel<KMAX, 8><<<grid, 128, 0, st>>>(a);
@@ -911,12 +927,14 @@ mm_status launch_adj_fused(const AdjArgs &a, cudaStream_t st)
     return check_launch("adjoint_fused_kernel");
 }
 
+// vox_end < 0: the whole volume; otherwise only voxels [vox_begin, vox_end) of `out` are written
 mm_status run_adjoint_fused(const mm_geometry *g, const float *B, const float *sino, int K, int ldk, int D,
-                            float *out, cudaStream_t st, int bilinear = 0)
+                            float *out, cudaStream_t st, int bilinear = 0, long long vox_begin = 0, long long vox_end = -1)
 {
     AdjArgs a;
     fill_adj(a, g, sino, B, out, K, ldk, D);
     a.bilinear = bilinear;
+    if (vox_end >= 0) { a.vox_begin = vox_begin; a.vox_end = vox_end; }
     a.vec_ok = (D % 4 == 0) && aligned16(sino);
     static const bool tc_off = getenv("MM_DISABLE_TC") != nullptr;     // debugging switch: CUDA-core contraction
     if (!tc_off && mm_adjoint_tc_supported(a)) {
@@ -1178,6 +1196,36 @@ extern "C" mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, 
     return check_launch("axpy_kernel");
 }
 
+// Device workspace of the host-buffer call: one grow-only arena and one stream per process, kept between calls
+// (cudaMalloc/cudaFree of 7 GB cost 20-330 ms per call on config 5, more than the copies); mm_host_workspace_release
+// frees it.  Calls are serialised by the mutex.
+namespace {
+struct HostWorkspace {
+    std::mutex mu;
+    char *base = nullptr;
+    size_t bytes = 0;
+    cudaStream_t stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t range_done = nullptr;
+    int device = -1;
+} g_hws;
+
+void hws_free_locked()
+{
+    if (g_hws.base) cudaFree(g_hws.base);
+    if (g_hws.stream) cudaStreamDestroy(g_hws.stream);
+    if (g_hws.copy_stream) cudaStreamDestroy(g_hws.copy_stream);
+    if (g_hws.range_done) cudaEventDestroy(g_hws.range_done);
+    g_hws.base = nullptr; g_hws.bytes = 0; g_hws.stream = g_hws.copy_stream = nullptr; g_hws.range_done = nullptr; g_hws.device = -1;
+}
+}   // namespace
+
+extern "C" mm_status mm_host_workspace_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_hws.mu);
+    hws_free_locked();
+    return MM_OK;
+}
+
 extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K, int32_t ldk,
                                            int32_t D, const float *h_data, const float *h_weights, float *h_grad, double *h_loss)
 {
@@ -1188,9 +1236,8 @@ extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_
     const size_t nvol = (size_t)g->shape[0] * g->shape[1] * g->shape[2] * ldk * sizeof(float);
     const size_t nsino = (size_t)g->P * g->J * g->Kd * D * sizeof(float);
     const size_t nB = (size_t)g->P * K * D * sizeof(float);
-    float *dB = nullptr, *dvol = nullptr, *ddata = nullptr, *dw = nullptr, *dgrad = nullptr, *dwr = nullptr;
-    double *dloss = nullptr;
-    cudaStream_t cs = nullptr;
+    auto up = [](size_t n) { return (n + 255) & ~(size_t)255; };          // every buffer 256-byte aligned
+    const size_t need = 2 * up(nvol) + (h_weights ? 3 : 2) * up(nsino) + up(nB) + 256;
     mm_status rc = MM_OK;
     cudaError_t e = cudaSuccess;
 #define MM_TRY(call, code)                                                              \
@@ -1199,24 +1246,45 @@ extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_
         cudaGetLastError();                                                             \
         rc = code;                                                                      \
     }
-    MM_TRY(cudaStreamCreate(&cs), MM_ERR_CUDA);
-    MM_TRY(cudaMalloc((void **)&dB, nB), MM_ERR_ALLOC);
-    MM_TRY(cudaMalloc((void **)&dvol, nvol), MM_ERR_ALLOC);
-    MM_TRY(cudaMalloc((void **)&ddata, nsino), MM_ERR_ALLOC);
-    if (h_weights) MM_TRY(cudaMalloc((void **)&dw, nsino), MM_ERR_ALLOC);
-    MM_TRY(cudaMalloc((void **)&dgrad, nvol), MM_ERR_ALLOC);
-    MM_TRY(cudaMalloc((void **)&dwr, nsino), MM_ERR_ALLOC);
-    MM_TRY(cudaMalloc((void **)&dloss, sizeof(double)), MM_ERR_ALLOC);
+    std::lock_guard<std::mutex> lock(g_hws.mu);
+    int dev = -1;
+    MM_TRY(cudaGetDevice(&dev), MM_ERR_CUDA);
+    if (rc == MM_OK && (dev != g_hws.device || need > g_hws.bytes)) {
+        hws_free_locked();
+        MM_TRY(cudaMalloc((void **)&g_hws.base, need), MM_ERR_ALLOC);
+        MM_TRY(cudaStreamCreate(&g_hws.stream), MM_ERR_CUDA);
+        MM_TRY(cudaStreamCreate(&g_hws.copy_stream), MM_ERR_CUDA);
+        MM_TRY(cudaEventCreateWithFlags(&g_hws.range_done, cudaEventDisableTiming), MM_ERR_CUDA);
+        if (rc == MM_OK) { g_hws.bytes = need; g_hws.device = dev; } else hws_free_locked();
+    }
+    if (rc != MM_OK) return rc;
+    char *p = g_hws.base;
+    auto take = [&](size_t n) { char *q = p; p += up(n); return q; };
+    float *dvol = (float *)take(nvol), *dgrad = (float *)take(nvol), *ddata = (float *)take(nsino), *dwr = (float *)take(nsino);
+    float *dw = h_weights ? (float *)take(nsino) : nullptr, *dB = (float *)take(nB);
+    double *dloss = (double *)take(sizeof(double));
+    cudaStream_t cs = g_hws.stream;
     MM_TRY(cudaMemcpyAsync(dB, h_B, nB, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
     MM_TRY(cudaMemcpyAsync(dvol, h_vol, nvol, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
     MM_TRY(cudaMemcpyAsync(ddata, h_data, nsino, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
     if (h_weights) MM_TRY(cudaMemcpyAsync(dw, h_weights, nsino, cudaMemcpyHostToDevice, cs), MM_ERR_CUDA);
-    if (rc == MM_OK) rc = mm_loss_gradient(g, dB, dvol, K, ldk, D, ddata, dw, dgrad, dloss, dwr, cs);
-    MM_TRY(cudaMemcpyAsync(h_grad, dgrad, nvol, cudaMemcpyDeviceToHost, cs), MM_ERR_CUDA);
+    if (rc == MM_OK) rc = run_residual_loss(g, dB, dvol, K, ldk, D, ddata, dw, dwr, dloss, cs, "mm_loss_gradient_host");   // phase 1
     MM_TRY(cudaMemcpyAsync(h_loss, dloss, sizeof(double), cudaMemcpyDeviceToHost, cs), MM_ERR_CUDA);
-    MM_TRY(cudaStreamSynchronize(cs), MM_ERR_CUDA);
+    // phase 2 in ranges of voxels: the device->host copy of a finished range runs on the copy stream under the
+    // next range's kernel (the 3.2 GB gradient of config 5 takes ~60 ms to copy, the kernel 123 ms)
+    const long long nvox = (long long)g->shape[0] * g->shape[1] * g->shape[2];
+    const int nrange = nvox >= 4096 ? 8 : 1;
+    cudaStream_t cp = g_hws.copy_stream;
+    for (int c = 0; c < nrange && rc == MM_OK; c++) {
+        const long long b = (nvox * c / nrange) & ~127LL, e2 = (c + 1 == nrange) ? nvox : ((nvox * (c + 1) / nrange) & ~127LL);
+        rc = run_adjoint_fused(g, dB, dwr, K, ldk, D, dgrad, cs, 0, b, e2);
+        MM_TRY(cudaEventRecord(g_hws.range_done, cs), MM_ERR_CUDA);
+        MM_TRY(cudaStreamWaitEvent(cp, g_hws.range_done, 0), MM_ERR_CUDA);
+        MM_TRY(cudaMemcpyAsync(h_grad + b * ldk, dgrad + b * ldk, (size_t)(e2 - b) * ldk * sizeof(float), cudaMemcpyDeviceToHost, cp),
+               MM_ERR_CUDA);
+    }
+    if (rc == MM_OK) { MM_TRY(cudaStreamSynchronize(cs), MM_ERR_CUDA); } else cudaStreamSynchronize(cs);
+    if (rc == MM_OK) { MM_TRY(cudaStreamSynchronize(cp), MM_ERR_CUDA); } else cudaStreamSynchronize(cp);
 #undef MM_TRY
-    cudaFree(dB); cudaFree(dvol); cudaFree(ddata); cudaFree(dw); cudaFree(dgrad); cudaFree(dwr); cudaFree(dloss);
-    if (cs) cudaStreamDestroy(cs);
     return rc;
 }

@@ -19,7 +19,7 @@ _lib = None
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
-           "mm_axpy_precond", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_launch_count", "mm_set_phase_event",
+           "mm_axpy_precond", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -72,6 +72,7 @@ def load():
     L.mm_nesterov_step.argtypes = [vp, vp, vp, ctypes.c_float, ctypes.c_float, i64, vp]
     L.mm_axpy_precond.argtypes = [vp, vp, vp, ctypes.c_float, i64, vp]
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
+    L.mm_host_workspace_release.argtypes = []
     L.mm_set_phase_event.argtypes = [vp]
     L.mm_launch_count.restype = i64
     L.mm_launch_count.argtypes = []
@@ -350,6 +351,11 @@ def _host(a, shape, who):
     if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous and a.shape == tuple(shape)):
         raise MMError(f"{who}: expected a C-contiguous float32 array of shape {tuple(shape)}")
     return ctypes.c_void_p(a.ctypes.data)
+
+
+def mm_host_workspace_release():
+    """Free the library-owned device workspace of mm_loss_gradient_host (it is kept between calls)."""
+    _check(load().mm_host_workspace_release(), "mm_host_workspace_release")
 
 
 def mm_loss_gradient_host(g: Geometry, h_B, h_vol, K: int, h_data, h_weights, h_grad):
