@@ -46,6 +46,9 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
 #ifndef FWD_MINB8
 #define FWD_MINB8 2                     // resident blocks per SM asked of the compiler for 32-byte lanes
 #endif
+#ifndef FWD_MIX48
+#define FWD_MIX48 1
+#endif
 #ifndef FWD_TK
 #define FWD_TK 4                        // rays along k in the tile of a 32-ray block
 #endif
@@ -164,6 +167,14 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     const int tid = threadIdx.x;
     const int q = tid % G;                        // lane within the ray's group
     const int r = tid / G;                        // ray within the block
+    // MIX (ldk = 48 only): lane q owns channels 8q..8q+7 (one 32-byte load) and 32+4q..32+4q+3 (one 16-byte load),
+    // so a warp's request touches each 192-byte record in a 128-byte and a 64-byte piece: 2.5 cache lines per
+    // tap on average against 3 for three 64-byte pieces (a load costs one L1 wavefront per distinct line).
+    constexpr bool MIX = FWD_MIX48 && VEC == 4 && G == 4 && NQ == 3;
+    auto chan = [&](int t) -> int {               // first channel of accumulator vector t of this lane
+        if constexpr (MIX) return t < 2 ? 8 * q + 4 * t : 32 + 4 * q;
+        else return VEC * (q + G * t);
+    };
     const int tiles_k = (a.Kd + TK - 1) / TK, tiles_j = (a.J + TJ - 1) / TJ;
     // Block order: FWD_GS consecutive projections (neighbouring rotation angles) are interleaved tile by tile, so
     // blocks resident at the same time walk the same band of the volume for several projections and the second
@@ -261,18 +272,34 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                     o[uu] = tap_o[r][i + uu];
                     w[uu] = tap_w[r][i + uu];
                 }
+                if constexpr (MIX) {
+                    const float *base = a.vol + 8 * q, *base2 = a.vol + 32 + 4 * q;
 #pragma unroll
-                for (int t = 0; t < NQ; t++) {
-                    // lanes past the last float4 of the voxel re-read its last one (same cache line, result
-                    // discarded in the epilogue): no branch in the loop
-                    const int e = min(q + G * t, ldk4 - 1);
-                    float c[U][4][VEC];
+                    for (int h = 0; h < U; h += 2) {              // 32-byte pieces, two slabs at a time
+                        float c[2][4][8];
+#pragma unroll
+                        for (int uu = 0; uu < 2; uu++) {
+                            ldg_nc_vec<8>(base + (long long)o[h + uu].x * 4, c[uu][0]);
+                            ldg_nc_vec<8>(base + (long long)o[h + uu].y * 4, c[uu][1]);
+                            ldg_nc_vec<8>(base + (long long)o[h + uu].z * 4, c[uu][2]);
+                            ldg_nc_vec<8>(base + (long long)o[h + uu].w * 4, c[uu][3]);
+                        }
+#pragma unroll
+                        for (int uu = 0; uu < 2; uu++) {
+                            const float ww[4] = {w[h + uu].x, w[h + uu].y, w[h + uu].z, w[h + uu].w};
+#pragma unroll
+                            for (int p = 0; p < 4; p++)
+#pragma unroll
+                                for (int x = 0; x < 8; x++) acc[x / 4][x % 4] = fmaf(ww[p], c[uu][p][x], acc[x / 4][x % 4]);
+                        }
+                    }
+                    float c[U][4][4];                             // 16-byte pieces
 #pragma unroll
                     for (int uu = 0; uu < U; uu++) {
-                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].x + e) * VEC, c[uu][0]);
-                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].y + e) * VEC, c[uu][1]);
-                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].z + e) * VEC, c[uu][2]);
-                        ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].w + e) * VEC, c[uu][3]);
+                        ldg_nc_vec<4>(base2 + (long long)o[uu].x * 4, c[uu][0]);
+                        ldg_nc_vec<4>(base2 + (long long)o[uu].y * 4, c[uu][1]);
+                        ldg_nc_vec<4>(base2 + (long long)o[uu].z * 4, c[uu][2]);
+                        ldg_nc_vec<4>(base2 + (long long)o[uu].w * 4, c[uu][3]);
                     }
 #pragma unroll
                     for (int uu = 0; uu < U; uu++) {
@@ -280,7 +307,30 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
 #pragma unroll
                         for (int p = 0; p < 4; p++)
 #pragma unroll
-                            for (int x = 0; x < VEC; x++) acc[t][x] = fmaf(ww[p], c[uu][p][x], acc[t][x]);
+                            for (int x = 0; x < 4; x++) acc[2][x] = fmaf(ww[p], c[uu][p][x], acc[2][x]);
+                    }
+                } else {
+    #pragma unroll
+                    for (int t = 0; t < NQ; t++) {
+                        // lanes past the last float4 of the voxel re-read its last one (same cache line, result
+                        // discarded in the epilogue): no branch in the loop
+                        const int e = min(q + G * t, ldk4 - 1);
+                        float c[U][4][VEC];
+    #pragma unroll
+                        for (int uu = 0; uu < U; uu++) {
+                            ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].x + e) * VEC, c[uu][0]);
+                            ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].y + e) * VEC, c[uu][1]);
+                            ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].z + e) * VEC, c[uu][2]);
+                            ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].w + e) * VEC, c[uu][3]);
+                        }
+    #pragma unroll
+                        for (int uu = 0; uu < U; uu++) {
+                            const float ww[4] = {w[uu].x, w[uu].y, w[uu].z, w[uu].w};
+    #pragma unroll
+                            for (int p = 0; p < 4; p++)
+    #pragma unroll
+                                for (int x = 0; x < VEC; x++) acc[t][x] = fmaf(ww[p], c[uu][p][x], acc[t][x]);
+                        }
                     }
                 }
             }
@@ -308,12 +358,12 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
             const float *p00 = slab + (long long)iu * sU + (long long)iv * sV;
 #pragma unroll
             for (int t = 0; t < NQ; t++) {
-                const int e = q + G * t;
-                if (VEC * e < a.ldk) {
+                const int ch = chan(t);
+                if (ch < a.ldk) {
                     float c00[VEC], c10[VEC], c01[VEC], c11[VEC];
 #pragma unroll
                     for (int x = 0; x < VEC; x++) c00[x] = c10[x] = c01[x] = c11[x] = 0.f;
-                    const float *pe = p00 + VEC * e;
+                    const float *pe = p00 + ch;
                     if (u0 && v0) Ld<VEC>::ld(pe, c00);
                     if (u1 && v0) Ld<VEC>::ld(pe + sU, c10);
                     if (u0 && v1) Ld<VEC>::ld(pe + sV, c01);
@@ -337,12 +387,12 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         if (!ray_ok) return;
 #pragma unroll
         for (int t = 0; t < NQ; t++) {
-            const int e = q + G * t;
-            if (VEC * e < a.ldk) {
+            const int ch = chan(t);
+            if (ch < a.ldk) {
                 float o[VEC];
 #pragma unroll
-                for (int x = 0; x < VEC; x++) o[x] = (VEC * e + x < a.K) ? w * acc[t][x] : 0.f;
-                Ld<VEC>::st(a.proj + ray * a.ldk + VEC * e, o);
+                for (int x = 0; x < VEC; x++) o[x] = (ch + x < a.K) ? w * acc[t][x] : 0.f;
+                Ld<VEC>::st(a.proj + ray * a.ldk + ch, o);
             }
         }
         return;
@@ -355,10 +405,10 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     const float *Bs = a.B + (long long)s * a.K * a.D;
 #pragma unroll
     for (int t = 0; t < NQ; t++) {
-        const int e = q + G * t;
+        const int ch = chan(t);
 #pragma unroll
         for (int x = 0; x < VEC; x++) {
-            const int i = VEC * e + x;
+            const int i = ch + x;
             if (i < a.K) {
                 const float pv_ = w * acc[t][x];
 #pragma unroll
@@ -855,7 +905,7 @@ mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
     // 48 floats per voxel (K = 45, configs 3 and 5) = 12 float4 = 4 lanes x 3: every lane's load is used.  The
     // 8 x 32-byte layout below would idle 2 lanes in 8, and the register write-back of a load costs the same
     // 8 wavefronts whether or not its lanes carry new data (profiles/r01_ncu_c5_v5.md): 198 -> 191 ms on config 5.
-    if (vec && a.ldk == 48) { launch_fwd<4, 4, 3, DMAX, MODE>(a, st); return check_launch("john_forward_kernel"); }
+    if (vec && a.ldk == 48 && (!FWD_MIX48 || (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0)) { launch_fwd<4, 4, 3, DMAX, MODE>(a, st); return check_launch("john_forward_kernel"); }
     // 32-byte lanes (LDG.E.256): 4 lanes cover up to 32 channels, 8 lanes up to 64, 16 lanes up to 128
     if (vec && a.ldk % 8 == 0 && a.ldk >= 24 && a.ldk <= 128 && (reinterpret_cast<uintptr_t>(a.vol) & 31u) == 0 &&
         (reinterpret_cast<uintptr_t>(a.proj) & 31u) == 0) {
