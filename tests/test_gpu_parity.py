@@ -315,6 +315,29 @@ def test_host_entry_point_matches_device_path(ora, mm):
     assert abs(L - Lo) <= TOL_LOSS * abs(Lo) and einf(h_grad[..., :c.K], go_grad) <= TOL
 
 
+def test_host_entry_point_arena_regrows_and_releases(ora, mm):
+    """The library-owned device arena of mm_loss_gradient_host is reused, regrown for a larger problem and freed by
+    mm_host_workspace_release; every call equals the device path bit for bit (8 voxel ranges, ragged last one)."""
+    import torch
+    for n, (shape, det, seed) in enumerate((((12, 10, 14), (15, 17), 3), ((33, 31, 29), (37, 35), 4), ((12, 10, 14), (15, 17), 3))):
+        cfg, c = cfg_case("C3", shape, det, 4, seed=seed)
+        _, gm = c.geoms(ora, mm)
+        B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(c.D))
+        data = synth.surrogate_model(cfg)
+        h_grad = np.full(gm.vol_shape(c.ldk), np.nan, dtype=np.float32)
+        L = mm.mm_loss_gradient_host(gm, B, c.vol, c.K, data, c.w, h_grad)
+        grad = torch.empty(gm.vol_shape(c.ldk), device="cuda")
+        loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+        wr = torch.empty(gm.proj_shape(c.D), device="cuda")
+        mm.mm_loss_gradient(gm, dev(B), dev(c.vol), c.K, dev(data), dev(c.w), grad, loss, wr)
+        assert abs(L - loss.item()) <= 1e-12 * abs(L)
+        assert np.array_equal(h_grad, grad.cpu().numpy())
+        if n == 1:
+            mm.mm_host_workspace_release()
+    mm.mm_host_workspace_release()
+    mm.mm_host_workspace_release()          # idempotent
+
+
 def test_gd_iterations_c4_recipe(ora, mm):
     """config 4's timed loop (gradient + fixed-step update) on a shrunk plate: trajectory parity."""
     import torch

@@ -185,3 +185,9 @@ def test_sh_matrix_full_two_theta_matches_oracle(mm, ora):
         got = mm.mm_basis_sh_matrix(gm, 6, s0, s1, two_theta=tt)
         assert np.abs(got - ora.basis_matrix(go, 6, s0, s1, two_theta=tt)).max() < 1e-6
     assert np.array_equal(mm.mm_basis_sh_matrix(gm, 6, s0, s1, two_theta=0.0), mm.mm_basis_sh_matrix(gm, 6, s0, s1))
+
+
+def test_host_workspace_release_with_nothing_allocated(mm):
+    """mm_host_workspace_release is a no-op (MM_OK) before any host call and needs no device."""
+    mm.mm_host_workspace_release()
+    mm.mm_host_workspace_release()
