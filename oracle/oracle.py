@@ -321,10 +321,11 @@ def adjoint(g: Geometry, B, sino, form="gather", threads=None):
     return john_adjoint(g, basis_adjoint(B, sino), form=form, threads=threads)
 
 
-def loss_gradient(g: Geometry, B, vol, data, weights=None, form="gather", threads=None):
+def loss_gradient(g: Geometry, B, vol, data, weights=None, form="gather", threads=None, model=None):
     """r = A c - I (Eq. 13); L = 1/2 sum w r^2 (Eq. 9 with a = 2, readings S10/S11); grad = A^T (w r).
-    Returns (L, grad[X][Y][Z][K], wr[P][J][Kd][D])."""
-    r = forward(g, B, vol, threads) - np.asarray(data, dtype=np.float64)
+    Returns (L, grad[X][Y][Z][K], wr[P][J][Kd][D]).  `model`: forward(g, B, vol) if the caller already holds it
+    (the large parity cases draw their data from it and must not pay for the forward twice)."""
+    r = (forward(g, B, vol, threads) if model is None else np.asarray(model, dtype=np.float64)) - np.asarray(data, dtype=np.float64)
     w = np.ones_like(r) if weights is None else np.asarray(weights, dtype=np.float64)
     wr = w * r
     L = 0.5 * float(np.sum(wr * r))

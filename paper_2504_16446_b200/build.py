@@ -1,6 +1,7 @@
 """Build the CUDA library in-tree: paper_2504_16446_b200/csrc/*.cu -> paper_2504_16446_b200/libmm.so.
 
-nvcc cross-compiles for sm_100a without a GPU.  The .so is git-ignored but travels to the GPU box with gpurun.
+nvcc cross-compiles for sm_100a without a GPU.  Each .cu is compiled to an object under csrc/.obj/ (in parallel,
+only when it or a header changed), then linked.  The .so is git-ignored but travels to the GPU box with gpurun.
 Usage: python -m paper_2504_16446_b200.build [--force] [--verbose]
 """
 from __future__ import annotations
@@ -9,30 +10,51 @@ import glob
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libmm.so")
+OBJ = os.path.join(HERE, "csrc", ".obj")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC,-O2,-Wall",
+         "-I", os.path.join(ROOT, "include"), "-I", os.path.join(HERE, "csrc")]
 
 
 def sources():
     return sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
 
 
-def _deps():
-    return sources() + glob.glob(os.path.join(HERE, "csrc", "*.h")) + glob.glob(os.path.join(ROOT, "include", "*.h"))
+def _headers():
+    return glob.glob(os.path.join(HERE, "csrc", "*.h")) + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + \
+        glob.glob(os.path.join(ROOT, "include", "*.h"))
+
+
+def _obj(src):
+    return os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+
+
+def _compile(src, verbose):
+    cmd = [NVCC] + FLAGS + (["-Xptxas=-v"] if verbose else []) + ["-c", src, "-o", _obj(src)]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    return src, r.returncode, r.stdout + r.stderr
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
-        return LIB
-    cmd = [NVCC, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-           "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-I", os.path.join(ROOT, "include"),
-           "-I", os.path.join(HERE, "csrc"), "-o", LIB] + sources()
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    subprocess.check_call(cmd)
+    os.makedirs(OBJ, exist_ok=True)
+    hdr_time = max([os.path.getmtime(h) for h in _headers()] + [os.path.getmtime(__file__)])
+    stale = [s for s in sources()
+             if force or not os.path.exists(_obj(s)) or os.path.getmtime(_obj(s)) < max(os.path.getmtime(s), hdr_time)]
+    if stale:
+        with ThreadPoolExecutor(max_workers=min(len(stale), os.cpu_count() or 1)) as ex:
+            for src, rc, out in ex.map(lambda s: _compile(s, verbose), stale):
+                if out.strip() and (verbose or rc != 0):
+                    print(out, file=sys.stderr)
+                if rc != 0:
+                    raise RuntimeError(f"nvcc failed on {src}")
+    objs = [_obj(s) for s in sources()]
+    if stale or not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(o) for o in objs):
+        subprocess.check_call([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     return LIB
 
 

@@ -140,8 +140,9 @@ extern "C" mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometr
         t.Mkv = ba * (h.ks[v] - t.sv * h.ks[m]);
         t.Cu = xc[u] - t.su * xc[m] - (jc + dj) * t.Mju - (kc + dk) * t.Mku;
         t.Cv = xc[v] - t.sv * xc[m] - (jc + dj) * t.Mjv - (kc + dk) * t.Mkv;
-        t.su_fx = llrint(ldexp(t.su, 32));
-        t.sv_fx = llrint(ldexp(t.sv, 32));
+        t.su_fx = llrint(ldexp(t.su, 40));
+        t.sv_fx = llrint(ldexp(t.sv, 40));
+        t.w64 = h.w;
         // voxel -> detector: j0 = jc + dj + (a/b) js.(x - xc)
         t.Jc = jc + dj; t.Kc = kc + dk;
         for (int i = 0; i < 3; i++) {
@@ -154,7 +155,7 @@ extern "C" mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometr
         t.hj = (float)((fabs(t.Mkv) + fabs(t.Mku)) / fabs(det) * (1.0 + 1e-6) + 1e-6);
         t.hk = (float)((fabs(t.Mjv) + fabs(t.Mju)) / fabs(det) * (1.0 + 1e-6) + 1e-6);
         // half-width <= 1: at most 2 candidate rays along that detector axis; < 1.5: at most 3
-        t.gcode = (t.hj < 1.5f && t.hk < 1.5f) ? 4 + 2 * (t.hj <= 1.00002f ? 0 : 1) + (t.hk <= 1.00002f ? 0 : 1) : 1;
+        t.gcode = (t.hj < 1.5f && t.hk < 1.5f) ? 4 + 2 * (t.hj <= 1.000003f ? 0 : 1) + (t.hk <= 1.000003f ? 0 : 1) : 1;
         t.pad_ = 0;
     }
     // Upload the table.  On a machine without a CUDA device the geometry stays host-only (mm_geometry_get and

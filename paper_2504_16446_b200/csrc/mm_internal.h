@@ -13,7 +13,7 @@
 // Forward (ray-stationary Joseph; Eq. 4): ray (j,k) of projection s crosses
 // slab n of the major axis m at in-slab position
 //     pu = Cu + j*Mju + k*Mku + n*su,      pv = Cv + j*Mjv + k*Mkv + n*sv         (voxel units)
-// The kernels evaluate this in 32.32 fixed point (exact incremental adds along the ray), hence the *_fx
+// The kernels evaluate this in 24.40 fixed point (exact incremental adds along the ray), hence the *_fx
 // copies of the slopes.
 //
 // Adjoint (voxel-stationary gather): voxel (x,y,z) projects to detector position
@@ -32,7 +32,8 @@ struct MMProj {
     float w;                       // Joseph step a/|d_m|
     int gcode;                     // gather window: 1 = generic loop; 4 + 2*(NJ-2) + (NK-2) = fixed NJ x NK, NJ,NK in {2,3}
     // ---
-    long long su_fx, sv_fx;        // round(su * 2^32), round(sv * 2^32)
+    long long su_fx, sv_fx;        // round(su * 2^40), round(sv * 2^40)
+    double w64;                    // Joseph step a/|d_m| unrounded (forward epilogue)
     int m, u, v;                   // major axis and the two in-slab axes (u < v)
     int pad_;
 };

@@ -52,8 +52,12 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
 #ifndef FWD_TK
 #define FWD_TK 4                        // rays along k in the tile of a 32-ray block
 #endif
-#define FX_ONE 4294967296.0            // 2^32
-#define FX_INV 2.3283064365386963e-10f // 2^-32
+// In-slab ray positions in 24.40 fixed point: exact incremental adds along the ray, slope resolution 2^-41 voxel per
+// slab (2e-10 voxel over 256 slabs; 32.32 left 3e-8, a shear common to all rays of a projection and therefore a
+// coherent error in the residual).  Integer part = tap index, top 32 fraction bits -> bilinear weight.
+#define FX_BITS 40
+#define FX_ONE 1099511627776.0         // 2^40
+#define FX_INV 2.3283064365386963e-10f // 2^-32 (the weight is taken from the top 32 fraction bits)
 
 // ================================================================================================
 // forward: ray-stationary Joseph
@@ -199,11 +203,22 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     const long long sM = (m == 0) ? sX : (m == 1 ? sY : sZ);
     const long long sU = (u == 0) ? sX : sY, sV = (v == 2) ? sZ : sY;
 
+    // Accumulation: fp32 FMAs run over a short round of slabs only (4 taps x U slabs, starting from
+    // zero), then the round is added to an fp64 total.  A plain fp32 running sum over <= 256 slabs x 4 taps carries
+    // ~3e-7 of the ray sum in rounding, which the residual r = Ac - data (1 % of Ac at 1e4 counts) magnifies to
+    // ~3e-5 in the gradient; with short rounds the rounding is relative to the round's own partial sum (~1e-8).
     float acc[NQ][VEC];
+    double tot[NQ][VEC];
 #pragma unroll
     for (int t = 0; t < NQ; t++)
 #pragma unroll
-        for (int x = 0; x < VEC; x++) acc[t][x] = 0.f;
+        for (int x = 0; x < VEC; x++) { acc[t][x] = 0.f; tot[t][x] = 0.0; }
+    auto flush = [&]() {
+#pragma unroll
+        for (int t = 0; t < NQ; t++)
+#pragma unroll
+            for (int x = 0; x < VEC; x++) { tot[t][x] += (double)acc[t][x]; acc[t][x] = 0.f; }
+    };
 
     if constexpr (COOP) {
         static_assert(!COOP || VEC == 4 || VEC == 8, "cooperative march needs 16- or 32-byte lanes");
@@ -242,11 +257,11 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                 t.o00 = t.o10 = t.o01 = t.o11 = 0;
                 t.w00 = t.w10 = t.w01 = t.w11 = 0.f;
                 if (n <= n1) {
-                    // 32.32 fixed point: the integer part is the tap index, the fraction the bilinear weight
+                    // 24.40 fixed point: the integer part is the tap index, the fraction the bilinear weight
                     const long long pu = pu0 + (long long)n * su_fx, pv = pv0 + (long long)n * sv_fx;
-                    const int iu = (int)(pu >> 32), iv = (int)(pv >> 32);
-                    const float fu = (float)(unsigned int)(pu & 0xffffffffLL) * FX_INV;
-                    const float fv = (float)(unsigned int)(pv & 0xffffffffLL) * FX_INV;
+                    const int iu = (int)(pu >> FX_BITS), iv = (int)(pv >> FX_BITS);
+                    const float fu = (float)(unsigned int)(pu >> (FX_BITS - 32)) * FX_INV;
+                    const float fv = (float)(unsigned int)(pv >> (FX_BITS - 32)) * FX_INV;
                     const bool u0 = (unsigned)iu < (unsigned)Nu, u1 = (unsigned)(iu + 1) < (unsigned)Nu;
                     const bool v0 = (unsigned)iv < (unsigned)Nv, v1 = (unsigned)(iv + 1) < (unsigned)Nv;
                     const int b0 = n * sM4 + (u0 ? iu * sU4 : 0), b1 = n * sM4 + (u1 ? (iu + 1) * sU4 : 0);
@@ -284,6 +299,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                             ldg_nc_vec<8>(base + (long long)o[h + uu].z * 4, c[uu][2]);
                             ldg_nc_vec<8>(base + (long long)o[h + uu].w * 4, c[uu][3]);
                         }
+                        if (h == 0) flush();                      // the previous step's sums, under this step's load latency
 #pragma unroll
                         for (int uu = 0; uu < 2; uu++) {
                             const float ww[4] = {w[h + uu].x, w[h + uu].y, w[h + uu].z, w[h + uu].w};
@@ -323,6 +339,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                             ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].z + e) * VEC, c[uu][2]);
                             ldg_nc_vec<VEC>(a.vol + (long long)(o[uu].w + e) * VEC, c[uu][3]);
                         }
+                        if (t == 0) flush();                      // the previous step's sums, under this step's load latency
     #pragma unroll
                         for (int uu = 0; uu < U; uu++) {
                             const float ww[4] = {w[uu].x, w[uu].y, w[uu].z, w[uu].w};
@@ -336,6 +353,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
             }
             __syncwarp();
         }
+        flush();
     } else if (ray_ok) {
         const double Au = pg->Cu + (double)j * pg->Mju + (double)k * pg->Mku;
         const double Av = pg->Cv + (double)j * pg->Mjv + (double)k * pg->Mkv;
@@ -344,14 +362,14 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         clip_range(Av, pg->sv, Nv, lo, hi);
         const int n0 = (int)ceil(lo), n1 = (int)floor(hi);
         const long long su_fx = pg->su_fx, sv_fx = pg->sv_fx;
-        // 32.32 fixed point: the integer part is the tap index, the fraction the bilinear weight
+        // 24.40 fixed point: the integer part is the tap index, the fraction the bilinear weight
         long long pu = (long long)floor(Au * FX_ONE) + (long long)n0 * su_fx;
         long long pv = (long long)floor(Av * FX_ONE) + (long long)n0 * sv_fx;
         const float *slab = a.vol + (long long)n0 * sM;
         for (int n = n0; n <= n1; n++) {
-            const int iu = (int)(pu >> 32), iv = (int)(pv >> 32);
-            const float fu = (float)(unsigned int)(pu & 0xffffffffLL) * FX_INV;
-            const float fv = (float)(unsigned int)(pv & 0xffffffffLL) * FX_INV;
+            const int iu = (int)(pu >> FX_BITS), iv = (int)(pv >> FX_BITS);
+            const float fu = (float)(unsigned int)(pu >> (FX_BITS - 32)) * FX_INV;
+            const float fv = (float)(unsigned int)(pv >> (FX_BITS - 32)) * FX_INV;
             const bool u0 = (unsigned)iu < (unsigned)Nu, u1 = (unsigned)(iu + 1) < (unsigned)Nu;
             const bool v0 = (unsigned)iv < (unsigned)Nv, v1 = (unsigned)(iv + 1) < (unsigned)Nv;
             const float w00 = (1.f - fu) * (1.f - fv), w10 = fu * (1.f - fv), w01 = (1.f - fu) * fv, w11 = fu * fv;
@@ -378,9 +396,11 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                 }
             }
             pu += su_fx; pv += sv_fx; slab += sM;
+            if (((n - n0) & 7) == 7) flush();
         }
+        flush();
     }
-    const float w = pg->w;
+    const double w = pg->w64;                     // Joseph step a/|d_m| in fp64: its fp32 rounding is a per-projection scale error
     const long long ray = ((long long)s * a.J + j) * a.Kd + k;
 
     if constexpr (MODE == 0) {
@@ -391,7 +411,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
             if (ch < a.ldk) {
                 float o[VEC];
 #pragma unroll
-                for (int x = 0; x < VEC; x++) o[x] = (ch + x < a.K) ? w * acc[t][x] : 0.f;
+                for (int x = 0; x < VEC; x++) o[x] = (ch + x < a.K) ? (float)(w * tot[t][x]) : 0.f;
                 Ld<VEC>::st(a.proj + ray * a.ldk + ch, o);
             }
         }
@@ -399,9 +419,11 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     } else {
 
     // fused reciprocal-space map (Eq. 6): Imod[c] = sum_i B[s][i][c] p[i], reduced over the ray's G lanes
-    float part[DMAX];
+    // in fp64: 45 x 8 DFMA per ray, once per ray — nothing next to the march, and the residual below is then
+    // formed from an unrounded model value
+    double part[DMAX];
 #pragma unroll
-    for (int c = 0; c < DMAX; c++) part[c] = 0.f;
+    for (int c = 0; c < DMAX; c++) part[c] = 0.0;
     const float *Bs = a.B + (long long)s * a.K * a.D;
 #pragma unroll
     for (int t = 0; t < NQ; t++) {
@@ -410,10 +432,10 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         for (int x = 0; x < VEC; x++) {
             const int i = ch + x;
             if (i < a.K) {
-                const float pv_ = w * acc[t][x];
+                const double pv_ = w * tot[t][x];
 #pragma unroll
                 for (int c = 0; c < DMAX; c++)
-                    if (c < a.D) part[c] = fmaf(__ldg(Bs + (long long)i * a.D + c), pv_, part[c]);
+                    if (c < a.D) part[c] = fma((double)__ldg(Bs + (long long)i * a.D + c), pv_, part[c]);
             }
         }
     }
@@ -430,18 +452,18 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         if ((c % G) == q && c < a.D && ray_ok) {
             const long long o = ray * a.D + c;
             if (MODE == 1) {
-                a.sino[o] = part[c];
+                a.sino[o] = (float)part[c];
             } else {
-                const float res = part[c] - __ldg(a.data + o);            // r = Ac - I  (Eq. 13)
-                const float wt = a.weights ? __ldg(a.weights + o) : 1.f;
-                float psi = res;                                           // rho'(r): r, or clip(r, -delta, delta) (Huber, S23)
-                double rho = 0.5 * (double)res * (double)res;             // L = sum w rho(r): 1/2 r^2 (S10) ...
-                if (a.huber > 0.f && fabsf(res) > a.huber) {
-                    psi = copysignf(a.huber, res);
-                    rho = (double)a.huber * ((double)fabsf(res) - 0.5 * (double)a.huber);   // ... or delta (|r| - delta/2)
+                const double res = part[c] - (double)__ldg(a.data + o);   // r = Ac - I  (Eq. 13), unrounded model value
+                const double wt = a.weights ? (double)__ldg(a.weights + o) : 1.0;
+                double psi = res;                                          // rho'(r): r, or clip(r, -delta, delta) (Huber, S23)
+                double rho = 0.5 * res * res;                              // L = sum w rho(r): 1/2 r^2 (S10) ...
+                if (a.huber > 0.f && fabs(res) > (double)a.huber) {
+                    psi = copysign((double)a.huber, res);
+                    rho = (double)a.huber * (fabs(res) - 0.5 * (double)a.huber);   // ... or delta (|r| - delta/2)
                 }
-                a.sino[o] = wt * psi;
-                lsum += (double)wt * rho;
+                a.sino[o] = (float)(wt * psi);
+                lsum += wt * rho;
             }
         }
     }

@@ -276,13 +276,16 @@ def test_gpu_dot_product_identity(mm):
 
 
 def test_zero_residual_and_zero_weight(mm):
-    """data = A c gives L ~ 0, grad ~ 0; zero-weight pixels do not contribute (reading S11)."""
+    """data = A c (rounded to fp32, as any data is) gives L ~ 0, grad ~ 0: the residual is that rounding and nothing
+    else, because the model value is kept unrounded until the subtraction; zero-weight pixels do not
+    contribute whatever they hold (reading S11)."""
     import torch
     cfg = synth.get_config("C2", shape=(20, 20, 20), det=(22, 22), n_rot=3)
     rot, tilt = synth.angles(cfg)
     gm = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
     K, ldk, D = cfg.K, 16, cfg.D
-    B = dev(mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D)))
+    hB = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    B = dev(hB)
     vol = dev(synth.make_volume(cfg, ldk))
     model = torch.empty(gm.proj_shape(D), device="cuda")
     mm.mm_forward(gm, B, vol, K, model)
@@ -290,11 +293,18 @@ def test_zero_residual_and_zero_weight(mm):
     loss = torch.zeros(1, device="cuda", dtype=torch.float64)
     wr = torch.empty_like(model)
     mm.mm_loss_gradient(gm, B, vol, K, model, None, grad, loss, wr)
-    assert loss.item() == 0.0 and torch.all(grad == 0).item()
+    u = 2.0 ** -24
+    assert torch.all(wr.abs() <= 1.01 * u * model.abs()).item()
+    assert loss.item() <= 0.5 * float((u * model.double()).pow(2).sum())
+    bound = torch.empty_like(grad)
+    mm.mm_adjoint(gm, dev(np.abs(hB)), model.abs(), K, bound)             # |A|^T |model| bounds |A^T wr| / u entrywise
+    assert torch.all(grad.abs() <= 1.01 * u * bound + 1e-30).item()
     w = (torch.rand(gm.proj_shape(D), device="cuda") > 0.5).float()
     junk = model + 1e6 * (1 - w) * torch.randn_like(model)               # garbage where the weight is 0
+    g1, l1, w1 = torch.empty_like(grad), torch.zeros_like(loss), torch.empty_like(wr)
+    mm.mm_loss_gradient(gm, B, vol, K, model, w, g1, l1, w1)
     mm.mm_loss_gradient(gm, B, vol, K, junk, w, grad, loss, wr)
-    assert loss.item() == 0.0 and torch.all(grad == 0).item()
+    assert loss.item() == l1.item() and torch.equal(grad, g1) and torch.equal(wr, w1)
 
 
 def test_host_entry_point_matches_device_path(ora, mm):
