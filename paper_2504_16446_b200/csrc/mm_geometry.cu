@@ -2,6 +2,7 @@
 // basis-matrix helper (step a2).  All fp64, runs once per geometry.  Citations: P:NN = PAPER.md line NN.
 #include <cuda_runtime.h>
 #include <math.h>
+#include <algorithm>
 #include <string.h>
 
 #include <new>
@@ -157,6 +158,24 @@ extern "C" mm_status mm_geometry_create(const mm_geometry_desc *desc, mm_geometr
         // half-width <= 1: at most 2 candidate rays along that detector axis; < 1.5: at most 3
         t.gcode = (t.hj < 1.5f && t.hk < 1.5f) ? 4 + 2 * (t.hj <= 1.000003f ? 0 : 1) + (t.hk <= 1.000003f ? 0 : 1) : 1;
         t.pad_ = 0;
+    }
+    // Detector tile of the brick adjoint (mm_adjoint_brick.cu): a 4 x 4 x 8 brick of voxels spans
+    // ext = 3|Jx| + 3|Jy| + 7|Jz| pixels along j; with the tile origin two pixels below the nearest pixel of the lowest
+    // corner and 3-wide candidate windows the indices used are 0 .. floor(ext + 3) + 1.
+    g->brick_tj = g->brick_tk = 0;
+    {
+        int tj = 0, tk = 0;
+        bool ok = true;
+        for (int s = 0; s < P && ok; s++) {
+            const MMProj &t = g->table[s];
+            if (t.gcode < 4) { ok = false; break; }
+            const double ej = 3.0 * fabs(t.Jx[0]) + 3.0 * fabs(t.Jx[1]) + 7.0 * fabs(t.Jx[2]);
+            const double ek = 3.0 * fabs(t.Kx[0]) + 3.0 * fabs(t.Kx[1]) + 7.0 * fabs(t.Kx[2]);
+            tj = std::max(tj, (int)floor(ej + 3.0 + 1e-3) + 2);
+            tk = std::max(tk, (int)floor(ek + 3.0 + 1e-3) + 2);
+        }
+        tk |= 1;                                             // odd row pitch: rows start in different shared-memory banks
+        if (ok && tj <= 16 && tk <= 17) { g->brick_tj = tj; g->brick_tk = tk; }
     }
     // Upload the table.  On a machine without a CUDA device the geometry stays host-only (mm_geometry_get and
     // mm_basis_sh_matrix work; every device call then fails with MM_ERR_CUDA — there is no CPU fallback).

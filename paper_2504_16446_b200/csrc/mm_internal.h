@@ -6,6 +6,8 @@
 #include <string>
 #include <vector>
 
+#include <cuda_runtime.h>
+
 #include "mm.h"
 
 // Per-projection ray table entry, built on the host in fp64 (mm_geometry.cpp), read by every kernel.
@@ -55,6 +57,9 @@ struct mm_geometry {
     std::vector<MMProj> table;
     MMProj *d_table;               // device copy of `table`
     int device;
+    // detector tile (pixels) that holds every candidate ray of a 4x4x8 voxel brick, maximum over the projections;
+    // 0 if some projection needs the generic candidate window or a tile beyond 16 x 17 (mm_adjoint_brick.cu)
+    int brick_tj, brick_tk;
 };
 
 void mm_set_error(const std::string &msg);
@@ -71,6 +76,17 @@ struct AdjArgs {
     long long vox_begin, vox_end;   // fused kernels: voxels [vox_begin, vox_end) of the launch (whole volume by default)
     int bilinear;             // 0: exact transpose of the Joseph forward (S9); 1: the paper's bilinear back-projection
 };
+
+// mm_runtime.cu: stream-ordered scratch from the library's own memory pool; TMA tensor maps
+cudaError_t mm_scratch_alloc(void **p, size_t bytes, cudaStream_t st);
+cudaError_t mm_scratch_free(void *p, cudaStream_t st);
+void mm_scratch_trim();
+bool mm_tma_available();
+bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long long n[4], const unsigned box[4]);
+
+// mm_adjoint_brick.cu: fused adjoint, voxel bricks + TMA-staged detector tiles + tcgen05 (3xTF32), the primary path
+bool mm_adjoint_brick_supported(const mm_geometry *g, const AdjArgs &a);
+int mm_adjoint_brick_launch(const mm_geometry *g, const AdjArgs &a, void *stream);   // returns a cudaError_t
 
 // mm_adjoint_tc.cu: fused adjoint with the basis contraction on the tensor cores (tcgen05, 3xTF32).
 bool mm_adjoint_tc_supported(const AdjArgs &a);

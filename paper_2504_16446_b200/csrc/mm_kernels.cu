@@ -1009,6 +1009,17 @@ mm_status run_adjoint_fused(const mm_geometry *g, const float *B, const float *s
     if (vox_end >= 0) { a.vox_begin = vox_begin; a.vox_end = vox_end; }
     a.vec_ok = (D % 4 == 0) && aligned16(sino);
     static const bool tc_off = getenv("MM_DISABLE_TC") != nullptr;     // debugging switch: CUDA-core contraction
+    static const bool brick_off = getenv("MM_DISABLE_BRICK") != nullptr;   // debugging switch: round-1 global-load gather
+    if (!tc_off && !brick_off && mm_adjoint_brick_supported(g, a)) {   // primary path: bricks + TMA tiles + tcgen05
+        const cudaError_t e = (cudaError_t)mm_adjoint_brick_launch(g, a, st);
+        if (e != cudaSuccess) {
+            mm_set_error(std::string("adjoint_brick_kernel: ") + cudaGetErrorString(e));
+            cudaGetLastError();
+            return MM_ERR_CUDA;
+        }
+        g_launches.fetch_add(2);                                      // bop_prep_kernel + adjoint_brick_kernel
+        return MM_OK;
+    }
     if (!tc_off && mm_adjoint_tc_supported(a)) {
         const cudaError_t e = (cudaError_t)mm_adjoint_tc_launch(a, st);
         if (e != cudaSuccess) {
@@ -1298,6 +1309,16 @@ extern "C" mm_status mm_host_workspace_release(void)
     return MM_OK;
 }
 
+extern "C" mm_status mm_workspace_release(void)
+{
+    {
+        std::lock_guard<std::mutex> lock(g_hws.mu);
+        hws_free_locked();
+    }
+    mm_scratch_trim();
+    return MM_OK;
+}
+
 extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K, int32_t ldk,
                                            int32_t D, const float *h_data, const float *h_weights, float *h_grad, double *h_loss)
 {
@@ -1345,10 +1366,13 @@ extern "C" mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_
     // phase 2 in ranges of voxels: the device->host copy of a finished range runs on the copy stream under the
     // next range's kernel (the 3.2 GB gradient of config 5 takes ~60 ms to copy, the kernel 123 ms)
     const long long nvox = (long long)g->shape[0] * g->shape[1] * g->shape[2];
-    const int nrange = nvox >= 4096 ? 8 : 1;
+    const long long plane = (long long)g->shape[1] * g->shape[2];
+    const int X = g->shape[0];
+    const int nrange = X >= 32 ? 8 : 1;                                   // ranges of whole x-planes, multiples of 4 planes
     cudaStream_t cp = g_hws.copy_stream;
     for (int c = 0; c < nrange && rc == MM_OK; c++) {
-        const long long b = (nvox * c / nrange) & ~127LL, e2 = (c + 1 == nrange) ? nvox : ((nvox * (c + 1) / nrange) & ~127LL);
+        const long long b = (long long)((X * c / nrange) & ~3) * plane;
+        const long long e2 = (c + 1 == nrange) ? nvox : (long long)((X * (c + 1) / nrange) & ~3) * plane;
         rc = run_adjoint_fused(g, dB, dwr, K, ldk, D, dgrad, cs, 0, b, e2);
         MM_TRY(cudaEventRecord(g_hws.range_done, cs), MM_ERR_CUDA);
         MM_TRY(cudaStreamWaitEvent(cp, g_hws.range_done, 0), MM_ERR_CUDA);

@@ -304,7 +304,8 @@ def test_zero_residual_and_zero_weight(mm):
     g1, l1, w1 = torch.empty_like(grad), torch.zeros_like(loss), torch.empty_like(wr)
     mm.mm_loss_gradient(gm, B, vol, K, model, w, g1, l1, w1)
     mm.mm_loss_gradient(gm, B, vol, K, junk, w, grad, loss, wr)
-    assert loss.item() == l1.item() and torch.equal(grad, g1) and torch.equal(wr, w1)
+    # (the loss is summed with fp64 atomics in no fixed order: equal to rounding, not bit for bit)
+    assert abs(loss.item() - l1.item()) <= 1e-12 * l1.item() and torch.equal(grad, g1) and torch.equal(wr, w1)
 
 
 def test_host_entry_point_matches_device_path(ora, mm):
