@@ -13,6 +13,8 @@ What is here (numpy, fp64) and what it follows:
   john_backproject_bilinear / backproject_bilinear  the paper's own unmatched adjoint  PAPER.md:314 (NEXT-1)
   basis_matrix_grid    NN indicator / GK Gaussian-kernel basis sets on a grid of orientations   PAPER.md:240-246 (NEXT-2)
   laplacian / laplacian_regulariser / l2_regulariser / nesterov_step   regularisers, momentum   PAPER.md:336-340 (NEXT-3)
+  iterate              regularised Nesterov iteration with the relative-change stop rule   PAPER.md:262-264, 270-272 (NEXT-3, reading S25)
+  sparsify_basis       sparse approximation of the reciprocal-space map   PAPER.md:274 (NEXT-2, reading S26)
   l1_regulariser / huber_norm_regulariser / total_variation_regulariser   PAPER.md:336-338 (NEXT-3, reading S24)
   derived_quantities   mean, second-moment tensor, eigen-decomposition, FA   PAPER.md:198-224, Eq. 10-12 (NEXT-4)
   huber_loss_gradient  Huber-regressor loss and its gradient   PAPER.md:334 (NEXT-4, reading S23)
@@ -461,6 +463,62 @@ def nesterov_step(c, v, grad_at_lookahead, eta, momentum):
         v <- m v - eta g(c + m v);   c <- c + v.   Returns (c_new, v_new); the caller evaluates g at c + m v."""
     v_new = momentum * np.asarray(v, dtype=np.float64) - eta * np.asarray(grad_at_lookahead, dtype=np.float64)
     return np.asarray(c, dtype=np.float64) + v_new, v_new
+
+
+def iterate(g: Geometry, B, data, weights, c0, eta, momentum, mu_laplacian, mu_l2, max_iter, tol, check_every=1, threads=None):
+    """A regularised gradient iteration that runs until the relative change of the loss drops below `tol`
+    ("a stop criterion based on the relative change of the loss function"; PAPER.md:262 MITRA: arbitrary
+    regularisers + Nesterov momentum; the asynchronous pipelines keep this loop on the GPU).
+    Reading S25 (the paper gives no formulas): iteration k = 0, 1, ... evaluates everything at the look-ahead point
+    y_k = c_k + m v_k (reading S22),
+        L_k = 1/2 sum w r(y_k)^2 + mu_lap/2 ||Lap y_k||^2 + mu_l2/2 ||y_k||^2,      g_k = grad of that at y_k,
+        v_{k+1} = m v_k - eta g_k,   c_{k+1} = c_k + v_{k+1}                           (fp32 state, as the device holds it),
+    and after the update of every `check_every`-th iteration (k + 1 a multiple of check_every, k >= 1) stops if
+        |L_k - L_{k-1}| <= tol |L_k|.
+    Returns (c, v, [L_0 .. L_last])."""
+    c = np.asarray(c0, dtype=np.float32).copy()
+    v = np.zeros_like(c)
+    m32, eta32 = np.float32(momentum), np.float32(eta)
+    losses = []
+    for k in range(int(max_iter)):
+        look = (c.astype(np.float64) + float(m32) * v.astype(np.float64)).astype(np.float32)
+        L, grad, _ = loss_gradient(g, B, look, data, weights, form="scatter", threads=threads)
+        if mu_laplacian:
+            R, gr = laplacian_regulariser(look)
+            L, grad = L + float(np.float32(mu_laplacian)) * R, grad + float(np.float32(mu_laplacian)) * gr
+        if mu_l2:
+            R, gr = l2_regulariser(look)
+            L, grad = L + float(np.float32(mu_l2)) * R, grad + float(np.float32(mu_l2)) * gr
+        losses.append(L)
+        c64, v64 = nesterov_step(c, v, grad, float(eta32), float(m32))
+        c, v = c64.astype(np.float32), v64.astype(np.float32)
+        if k >= 1 and (k + 1) % int(check_every) == 0 and abs(losses[-1] - losses[-2]) <= tol * abs(losses[-1]):
+            break
+    return c, v, losses
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-2 (second half): sparse approximation of the reciprocal-space map, PAPER.md:274
+# ------------------------------------------------------------------------------------------------
+def sparsify_basis(B, n_keep):
+    """The "sparse approximation to the reciprocal-space mapping" of the sparse pipelines ("... such as
+    only mapping one basis function to each segment").  Reading S26 (no formula in the paper): for every projection s
+    and segment c keep the n_keep coefficients B[s][i][c] of largest magnitude (lowest i first among equals) and set
+    the others to zero.  The sparse forward model, adjoint and gradient are `forward`, `adjoint`, `loss_gradient` with
+    this matrix; n_keep >= K changes nothing."""
+    B = np.asarray(B)
+    P, K, D = B.shape
+    n_keep = int(n_keep)
+    if n_keep >= K:
+        return B.copy()
+    out = np.zeros_like(B)
+    for s in range(P):
+        for c in range(D):
+            col = np.abs(B[s, :, c].astype(np.float64))
+            order = sorted(range(K), key=lambda i: (-col[i], i))[:n_keep]
+            for i in order:
+                out[s, i, c] = B[s, i, c]
+    return out
 
 
 # ------------------------------------------------------------------------------------------------
