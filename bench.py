@@ -45,6 +45,50 @@ def algorithmic_bytes(cfg):
     return fwd, fused
 
 
+def source_sha16():
+    """hash of the kernel sources: ties a stored ncu traffic figure to the code it was measured on"""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", "*.cu*")) +
+                    glob.glob(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", "*.h"))):
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def record_traffic(csv_path, cfg_name, command):
+    """`--record-traffic`: read dram__bytes_{read,write}.sum per kernel from an `ncu --page raw --csv` export and store
+    them, with the hash of the kernel sources, in profiles/r02_traffic.json"""
+    import csv
+    with open(csv_path) as f:
+        rows = list(csv.reader(f))
+    hdr = rows[0]
+    ik, ir, iw = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    unit = {"Gbyte": 1e9, "Mbyte": 1e6, "Tbyte": 1e12, "Kbyte": 1e3, "byte": 1.0}
+    ent = {}
+    for r in rows[2:]:
+        if len(r) <= max(ir, iw):
+            continue
+        b = float(r[ir]) * unit[rows[1][ir]] + float(r[iw]) * unit[rows[1][iw]]
+        for key in ("john_forward_kernel", "adjoint_brick_kernel"):
+            if key in r[ik]:
+                ent[key + "_dram_bytes"] = int(b)
+    out = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    tr = {}
+    if os.path.exists(out):
+        with open(out) as f:
+            tr = json.load(f)
+    if tr.get("source_sha16") != source_sha16():
+        tr = {}
+    tr["source_sha16"] = source_sha16()
+    tr["command"] = command
+    tr[cfg_name] = ent
+    with open(out, "w") as f:
+        json.dump(tr, f, indent=1)
+    print(json.dumps(tr))
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -103,10 +147,28 @@ class ClockSampler:
 # reference arm / cpu_baseline: the oracle on a bounded sample
 # -------------------------------------------------------------------------------------------------
 def oracle_sample(cfg, n_sample_proj):
-    """stratified projection subset: full volume, full detector, n_sample_proj of the P projections."""
+    """stratified projection subset: full volume, full detector, n_sample_proj of the P projections — spread over the
+    tilts first (projections are tilt-major) with the rotation staggered from tilt to tilt, so that a sample of
+    n_tilts projections has one per tilt and sweeps the rotation range (all three major axes on configs 2-5)."""
     rot, tilt = synth.angles(cfg)
-    idx = np.unique(((np.arange(n_sample_proj) + 0.5) * cfg.P / n_sample_proj).astype(int))
+    n_t, n_r = len(cfg.tilts_deg), cfg.n_rot
+    n = int(max(1, min(cfg.P, n_sample_proj)))
+    if n >= cfg.P:
+        return rot, tilt, np.arange(cfg.P)
+    per_t = -(-n // n_t)                                   # samples per tilt (the last tilts may get one fewer)
+    idx = []
+    for i in range(n):
+        t, m = (i % n_t, i // n_t) if n >= n_t else ((i * n_t + n_t // 2) // n, 0)
+        r = int((m + 0.5) * n_r / per_t + (t * n_r) / (float(n_t) * per_t)) % n_r      # staggered from tilt to tilt
+        idx.append(t * n_r + r)
+    idx = np.unique(np.array(idx, dtype=int))
     return rot[idx], tilt[idx], idx
+
+
+def major_axes(go, n):
+    """how many of the n projections of an oracle geometry march along x, y, z"""
+    m = [go.get(s)[3] for s in range(n)]
+    return {"x": m.count(0), "y": m.count(1), "z": m.count(2)}
 
 
 def run_oracle_step(ora, go, B, vol, data, w, K):
@@ -127,26 +189,46 @@ def oracle_setup(cfg, n_sample_proj, vol=None):
     return ora, go, B, vol, data, idx
 
 
-def sample_size_for(cfg):
-    # ~10-30 s of single-core oracle work; measured ~0.5e9 tap-FMAs/s, 6e9 tap-FMAs per projection at C5
-    per_proj = cfg.det[0] * cfg.det[1] * max(cfg.shape) * 4 * cfg.K * 2
-    return int(max(1, min(cfg.P, 0.9e10 // per_proj)))
+def proj_seconds(cfg):
+    """estimated single-core oracle time of one projection's loss_gradient (forward + scatter adjoint): measured
+    ~1.0e9 tap-FMAs/s on the B200 boxes' hosts (config 5: 6e9 tap-FMAs, 5.9 s)"""
+    return cfg.det[0] * cfg.det[1] * max(cfg.shape) * 4 * cfg.K * 2 / 1.0e9
+
+
+def sample_size_for(cfg, budget_s=55.0):
+    """projections in the cpu_baseline sample: at least one per tilt where that fits the time budget (config 5: 9
+    projections, ~55 s on one core), the whole config when it is small"""
+    n = int(budget_s // max(proj_seconds(cfg), 1e-9))
+    return int(max(1, min(cfg.P, n)))
 
 
 def reference_arm(args, cfg):
+    """`--impl reference`: the oracle as it stands, one host core.  Every step marches a bounded sample of the workload
+    (whole volume and detector, a few projections) sized so that warm-up + steps end within a few minutes; successive
+    steps take successive members of the one-per-tilt stratified set, so a run covers all tilts and major axes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_s = sample_size_for(cfg)
-    ora, go, B, vol, data, idx = oracle_setup(cfg, n_s)
+    per_step = max(1, min(cfg.P, int((150.0 / max(1, args.steps + args.warmup)) // max(proj_seconds(cfg), 1e-9))))
+    pool_n = min(cfg.P, max(len(cfg.tilts_deg), per_step))
+    ora, go, B, vol, data, idx = oracle_setup(cfg, pool_n)
     K = cfg.K
-    for _ in range(args.warmup):
-        run_oracle_step(ora, go, B, vol[..., :K], data, None, K)
-    ts = [run_oracle_step(ora, go, B, vol[..., :K], data, None, K) for _ in range(args.steps)]
-    t = sum(ts) / len(ts)
-    vcp = cfg.n_voxels * K * len(idx)
+    groups = [np.arange(i, i + per_step) % len(idx) for i in range(0, len(idx), per_step)]
+
+    def step(i):
+        sel = np.unique(groups[i % len(groups)])
+        g1 = ora.Geometry(cfg.shape, cfg.det, go.rot[sel], go.tilt[sel])
+        return run_oracle_step(ora, g1, B[sel], vol[..., :K], data[sel], None, K), len(sel)
+
+    for i in range(args.warmup):
+        step(i)
+    res = [step(args.warmup + i) for i in range(args.steps)]
+    t = sum(r[0] for r in res) / len(res)
+    nproj = sum(r[1] for r in res) / len(res)
+    vcp = cfg.n_voxels * K * nproj
     val = vcp / t / 1e9
-    sample = f"{len(idx)} of {cfg.P} projections (indices {idx.tolist()}), full {cfg.shape} volume and {cfg.det} detector"
+    sample = (f"{nproj:g} of {cfg.P} projections per step, drawn in turn from the stratified set {idx.tolist()} (one per tilt; "
+              f"major axes {major_axes(go, len(idx))}), full {cfg.shape} volume and {cfg.det} detector")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -297,16 +379,28 @@ def ours(args, cfg):
     achieved = fwd_bytes / (fwd_ms * 1e-3) / 1e9
     roofline = {"kernel": "john_forward_kernel (phase 1 of mm_loss_gradient: Joseph march + basis + residual + loss)",
                 "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "ms_per_launch": fwd_ms,
+                "bound_note": "frac is the STREAMING MODEL (one volume pass per projection) against the HBM copy peak; ncu "
+                              "shows the kernel bound by the L1 data pipe (register write-back of the gathered taps), and "
+                              "cross-projection L2 reuse keeps real DRAM traffic below the model: see dram_frac",
+                "traffic": None, "dram_frac": None, "peak_source": peak_src, "ms_per_launch": fwd_ms,
                 "algorithmic_bytes_per_launch": fwd_bytes,
                 "model": "streaming: 4 B per voxel-channel-projection + sinogram write (SURVEY.md 8d)",
                 "fused_step": {"algorithmic_bytes": fused_bytes, "achieved": fused_bytes / (ms_step * 1e-3) / 1e9,
                                "frac": fused_bytes / (ms_step * 1e-3) / 1e9 / peak},
                 "adjoint_kernel_ms": adj_ms}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    # measured DRAM bytes of that kernel (one ncu --set full capture, profiles/r02_traffic.json, written by
+    # `bench.py --record-traffic <ncu raw csv>`); only trusted while the kernel sources are the ones it was measured on
+    traffic_file = os.path.join(ROOT, "profiles", "r02_traffic.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
-            roofline["traffic"] = json.load(f).get(cfg.name, {}).get("john_forward_kernel_dram_bytes")
+            tr = json.load(f)
+        ent = tr.get(cfg.name, {})
+        if tr.get("source_sha16") == source_sha16() and ent.get("john_forward_kernel_dram_bytes"):
+            roofline["traffic"] = ent["john_forward_kernel_dram_bytes"]
+            roofline["dram_frac"] = roofline["traffic"] / (fwd_ms * 1e-3) / 1e9 / peak
+            roofline["traffic_source"] = tr.get("command")
+        else:
+            roofline["traffic_source"] = "profiles/r02_traffic.json is stale (kernel sources changed since the capture): null"
 
     # ---- cpu_baseline: the oracle, single core, on a bounded projection sample of the same workload
     cpu = None
@@ -316,7 +410,8 @@ def ours(args, cfg):
         ora, go, Bo, _, data_s, idx = oracle_setup(cfg, n_s, vol=vol_np)
         t = run_oracle_step(ora, go, Bo, vol_np[..., :K], data_s, None, K)
         cpu = {"value": cfg.n_voxels * K * len(idx) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "seconds": t, "sample": f"{len(idx)} of {cfg.P} projections (indices {idx.tolist()}), full volume and detector",
+               "seconds": t, "sample": f"{len(idx)} of {cfg.P} projections (indices {idx.tolist()}: stratified over the tilts, "
+                                       f"major axes {major_axes(go, len(idx))}), full volume and detector",
                "host_cores_available": len(os.sched_getaffinity(0))}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -338,8 +433,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true", help="also time mm_backproject (outside the step)")
+    ap.add_argument("--record-traffic", metavar="NCU_RAW_CSV", help="store the kernels' DRAM bytes from an ncu raw-page csv and exit")
+    ap.add_argument("--traffic-command", default="ncu --set full --clock-control none -k regex:john_forward|adjoint_brick ... python bench.py --steps 1 --warmup 3 --no-cpu-baseline; ncu -i <rep> --page raw --csv")
     args = ap.parse_args()
     cfg = synth.get_config(args.config)
+    if args.record_traffic:
+        record_traffic(args.record_traffic, cfg.name, args.traffic_command)
+        return
     if args.impl == "reference":
         reference_arm(args, cfg)
     else:

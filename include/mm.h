@@ -25,7 +25,12 @@
  *     each other; the fast path needs ldk % 4 == 0 and 16-byte aligned bases, otherwise a slower scalar path
  *     runs (same results).  "HOST" pointers are ordinary host memory.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device calls only enqueue
- *     work on it: no hidden allocation, no synchronisation, outputs overwritten (never accumulated).
+ *     work on it: no synchronisation, outputs overwritten (never accumulated).  The only memory a device call
+ *     obtains itself is scratch from a memory pool the library owns (cudaMallocFromPoolAsync / cudaFreeAsync on
+ *     `stream`: stream-ordered, no synchronisation, re-entrant, cached between calls; mm_workspace_release()
+ *     returns it to the driver).
+ *   - Volumes and data must be finite: taps outside the volume and rays with zero weight may still be read and
+ *     multiplied by zero (a NaN there would spread).
  *   - mm_geometry is immutable after creation; calls on different streams may run concurrently.
  *   - Errors: NULL required pointer -> MM_ERR_NULL; K<1, ldk<K, D<1, D>MM_MAX_D, shape<1 -> MM_ERR_SHAPE;
  *     non-finite angle, non-orthonormal axes -> MM_ERR_VALUE; CUDA launch/alloc failures -> MM_ERR_CUDA /
@@ -217,6 +222,32 @@ mm_status mm_regulariser(const mm_geometry *g, int32_t kind, const float *vol, i
                          float *grad_out, double *value, void *stream);
 mm_status mm_nesterov_step(float *c, float *v, const float *grad, float eta, float momentum, int64_t n, void *stream);
 
+/* NEXT-3 — the whole regularised iteration on the device (MITRA = gradient descent with Nesterov momentum and
+ * regularisers, SIGTT "uses a stop criterion based on the relative change of the loss function"; the
+ * asynchronous pipelines keep the loop on the GPU).  Reading S25: iteration k = 0, 1, ... works at the look-ahead point
+ * y_k = c_k + m v_k,
+ *     L_k = 1/2 sum w (A y_k - data)^2 + mu_laplacian/2 ||Lap y_k||^2 + mu_l2/2 ||y_k||^2,   g_k = its gradient at y_k,
+ *     v_{k+1} = m v_k - eta g_k,    c_{k+1} = c_k + v_{k+1},
+ * and after the update of every check_every-th iteration (k + 1 a multiple of check_every, k >= 1) stops if
+ * |L_k - L_{k-1}| <= tol |L_k| (tol <= 0: never).  c, v [X][Y][Z][ldk] DEVICE, in/out (v = momentum state: zeros for a
+ * fresh start; channels K..ldk-1 are left alone); losses DEVICE double[max_iter], out (L_0 .. L_{n_iter-1}); n_iter HOST
+ * out = iterations done.  All work is enqueued on `stream`; per check the host reads one 4-byte flag and waits for
+ * the stream (the only synchronisation; with tol <= 0 the call is fully asynchronous).  Scratch (2 or 4 volumes and
+ * one sinogram) comes from the library's stream-ordered pool.  MM_ERR_VALUE for eta <= 0, negative momentum/weights,
+ * max_iter or check_every < 1. */
+typedef struct {
+    float eta;              /* step length                                                      */
+    float momentum;         /* Nesterov m, 0 = plain gradient descent                   */
+    float mu_laplacian;     /* weight of the Laplacian regulariser, 0 = off            */
+    float mu_l2;            /* weight of the L2Norm regulariser, 0 = off               */
+    int32_t max_iter;
+    int32_t check_every;
+    double tol;
+} mm_iterate_params;
+mm_status mm_iterate(const mm_geometry *g, const float *B, int32_t K, int32_t ldk, int32_t D, const float *data,
+                     const float *weights, const mm_iterate_params *params, float *c, float *v, double *losses,
+                     int32_t *n_iter, void *stream);
+
 /* Fixed-step gradient-descent update c <- c - eta * grad on n floats (GradientDescent); DEVICE. */
 mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *stream);
 
@@ -227,6 +258,10 @@ mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *strea
  * grows on demand, is reused by later calls and is freed by mm_host_workspace_release(); calls are serialised
  * inside the library.  MM_ERR_ALLOC if the arena cannot be allocated (nothing is left allocated then). */
 mm_status mm_host_workspace_release(void);
+/* Also returns to the driver the device memory cached in the library's stream-ordered scratch pool (see "stream"
+ * above): the adjoint's split operand tiles (P*ldk*D*8 bytes), the forward's repacked volume when ldk = 48 (one
+ * volume), mm_iterate's work arrays.  The pool refills on the next call that needs it. */
+mm_status mm_workspace_release(void);
 mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K,
                                 int32_t ldk, int32_t D, const float *h_data, const float *h_weights,
                                 float *h_grad, double *h_loss);

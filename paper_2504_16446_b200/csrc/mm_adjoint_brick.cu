@@ -33,7 +33,11 @@ using namespace mmptx;
 
 namespace {
 
-constexpr int BX = 4, BY = 4, BZ = 8;              // brick; thread t: dz = t & 7, dy = (t >> 3) & 3, dx = t >> 5 (= warp)
+// brick of voxels per CTA; thread t = 32 warp + lane holds voxel (dx, dy, dz) = (lane bit 2 | warp bit 1 << 1,
+// lane bit 1 | warp bit 0 << 1, lane bit 0 | lane bits 3-4 << 1): the eight lanes of a quarter-warp (one shared-memory
+// access phase) form a 2 x 2 x 2 cube, whose shadow on the detector spans at most 3 x 3 pixels — pixel indices that the
+// swizzled tile keeps in different banks
+constexpr int BX = 4, BY = 4, BZ = 8;
 constexpr int NTHREADS = 192;
 constexpr int NST = 4;                             // tile ring depth
 constexpr int WIN_MMAS = 48;                       // MMAs per accumulation window (see drain_window)
@@ -69,24 +73,45 @@ struct Cfg {
     static_assert(USED <= 512, "tensor memory");
 };
 
-__device__ __forceinline__ float4 lds128(uint32_t addr)
+// two adjacent floats as one 64-bit register pair: sm_100 has packed fp32 arithmetic (fma.rn.f32x2 -> FFMA2), which
+// halves the issue slots of the gather's multiply-adds
+typedef unsigned long long f32x2;
+__device__ __forceinline__ void lds_2x2(uint32_t addr, f32x2 &a, f32x2 &b)
 {
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-    return v;
+    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
 }
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void fma2(f32x2 &acc, f32x2 w, f32x2 v) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(w), "l"(v)); }
 
-// t[c] += w * tile[addr + 4 c].  About half of the candidates of a window have zero weight; with SKIP their lanes
-// read a block of zeros instead (one address for all of them: a broadcast, no bank conflicts, one wavefront at most).
+// t[c] += w * tile[addr + 4 c] (t as D/2 packed pairs).  About half of the candidates of a window have zero weight;
+// with SKIP their lanes read a block of zeros instead (one address for all of them: a broadcast).
+//
+// The tile sits in shared memory with TMA's swizzle of one pixel's width (32 bytes for D = 8, 64 for D = 16): the low
+// bit(s) of the 16-byte chunk index (address bits 4..) are XORed with the low bit(s) of the 128-byte row index (bits
+// 7..).  Unswizzled, the eight lanes of a quarter-warp could use only four of the eight 16-byte bank groups (all lanes
+// read the same chunk of their pixel): every tile read was a 2-way conflict (ncu, round-2 v1: 91 wavefronts per warp
+// and projection against 47 ideal, L1 data pipe at 87 %).  Swizzled, lanes whose pixel indices differ mod 8 never collide.
 template <int D, bool SKIP>
-__device__ __forceinline__ void acc_candidate(float w, uint32_t addr, uint32_t zeros, float (&t)[D])
+__device__ __forceinline__ void acc_candidate(float w, uint32_t addr, uint32_t zeros, f32x2 (&t)[D / 2])
 {
     static_assert(D == 8 || D == 16, "D");
+    addr ^= (addr >> 3) & (D == 8 ? 0x10u : 0x30u);                  // a pixel never straddles a 128-byte row
     if (SKIP) addr = w > 0.f ? addr : zeros;
+    const f32x2 w2 = pack2(w, w);
 #pragma unroll
     for (int c = 0; c < D; c += 4) {
-        const float4 v = lds128(addr + 4 * c);
-        t[c] = fmaf(w, v.x, t[c]); t[c + 1] = fmaf(w, v.y, t[c + 1]); t[c + 2] = fmaf(w, v.z, t[c + 2]); t[c + 3] = fmaf(w, v.w, t[c + 3]);
+        // chunk c/4 of the pixel: the pixel is aligned to its size, so adding 4c bytes to the unswizzled address only
+        // sets low chunk-index bits that are zero there — the same as XORing them into the swizzled address
+        f32x2 a, b;
+        lds_2x2(addr ^ (uint32_t)(4 * c), a, b);
+        fma2(t[c / 2], w2, a);
+        fma2(t[c / 2 + 1], w2, b);
     }
 }
 
@@ -97,7 +122,7 @@ __device__ __forceinline__ void acc_candidate(float w, uint32_t addr, uint32_t z
 //   3-wide: integers within 1.5 of l are {n-1, n, n+1}, n = round(l);  2-wide: within 1 of l are {floor l, floor l + 1}.
 template <int D, int NJ, int NK, bool SKIP>
 __device__ __forceinline__ void gather_tile(const float4 cj, const float4 ck, const float4 cm, uint32_t tile, int pitch, uint32_t bias,
-                                            uint32_t zeros, float dxf, float dyf, float dzf, float (&t)[D])
+                                            uint32_t zeros, float dxf, float dyf, float dzf, f32x2 (&t)[D / 2])
 {
     // cj = (Jx0, Jx1, Jx2, base_lj), ck = (Kx0, Kx1, Kx2, base_lk), cm = (mju, mku, mjv, mkv)
     const float lj = fmaf(dxf, cj.x, fmaf(dyf, cj.y, fmaf(dzf, cj.z, cj.w)));
@@ -124,8 +149,11 @@ __device__ __forceinline__ void gather_tile(const float4 cj, const float4 ck, co
     }
 }
 
+// SKIP = 1 redirects the reads of zero-weight candidates to a block of zeros.  Measured on config 5 with the cube lane
+// mapping and the swizzled tile: 62.5 ms with, 57.1 ms without (the select costs more issue slots than the saved
+// wavefronts are worth once the reads are conflict-free); kept as a compile-time switch.
 #ifndef MM_BRICK_SKIP
-#define MM_BRICK_SKIP 1
+#define MM_BRICK_SKIP 0
 #endif
 
 template <int D, int NPAD>
@@ -136,15 +164,16 @@ adjoint_brick_kernel(const __grid_constant__ CUtensorMap tmap, const BrickArgs a
     constexpr int WIN = C::WIN;
     constexpr uint32_t IDESC = idesc_tf32(128, NPAD);
     extern __shared__ __align__(1024) unsigned char smem[];
-    // [tiles NST x tile_stride][B operands NST x BOP_BYTES][stage constants NST x 64][barriers][tmem slot]
+    // [tiles NST x tile_stride][B operands NST x BOP_BYTES][stage constants NST x 64][64 zero bytes][barriers][tmem slot]
     const uint32_t s_tiles = smem_u32(smem);
     const uint32_t s_bop = s_tiles + NST * a.tile_stride;
-    float4 *cst = reinterpret_cast<float4 *>(smem + NST * a.tile_stride + NST * C::BOP_BYTES);
-    const uint32_t s_bar = smem_u32(cst + 4 * NST);
+    unsigned char *tail = smem + NST * a.tile_stride + NST * C::BOP_BYTES;
+    float4 *cst = reinterpret_cast<float4 *>(tail);
+    float *zero_block = reinterpret_cast<float *>(tail + NST * 64);  // 64-byte aligned block of zeros (see acc_candidate)
+    const uint32_t s_bar = smem_u32(tail + NST * 64 + 64);
     const uint32_t full_tile = s_bar, empty_tile = s_bar + 8 * NST, full_a = s_bar + 16 * NST, empty_a = full_a + 16,
                    wbar = full_a + 32, drained = full_a + 40;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + NST * a.tile_stride + NST * C::BOP_BYTES + NST * 64 + 16 * NST + 48);
-    float *zero_block = reinterpret_cast<float *>(tmem_slot + 4);    // 64 bytes of zeros (see acc_candidate)
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tail + NST * 64 + 64 + 16 * NST + 48);
     constexpr bool SKIP = MM_BRICK_SKIP != 0;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -161,7 +190,7 @@ adjoint_brick_kernel(const __grid_constant__ CUtensorMap tmap, const BrickArgs a
         mbar_init(wbar, 1); mbar_init(drained, 4);
         mbar_fence_init();
     }
-    if ((s_tiles & 127u) != 0) __trap();                             // TMA destinations need 128-byte alignment
+    if ((s_tiles & 1023u) != 0) __trap();                            // swizzled TMA destinations need 1024-byte alignment
     if (tid == 128) tma_prefetch_desc(&tmap);
     if (tid < 16) zero_block[tid] = 0.f;
     tc_fence_before();
@@ -230,7 +259,7 @@ adjoint_brick_kernel(const __grid_constant__ CUtensorMap tmap, const BrickArgs a
         __syncwarp();
     } else {
         // ---------------- gather warps ----------------
-        const int dz = tid & 7, dy = (tid >> 3) & 3, dx = tid >> 5;
+        const int dz = (lane & 1) | ((lane >> 3) << 1), dy = ((lane >> 1) & 1) | ((warp & 1) << 1), dx = ((lane >> 2) & 1) | ((warp >> 1) << 1);
         const float dxf = (float)dx, dyf = (float)dy, dzf = (float)dz;
         const int pitch = a.tk * D * 4;
         const uint32_t bias = MAGIC_BITS * (uint32_t)pitch + MAGIC_BITS * (uint32_t)(D * 4);
@@ -271,15 +300,18 @@ adjoint_brick_kernel(const __grid_constant__ CUtensorMap tmap, const BrickArgs a
             const float4 cj = cst[4 * st], ck = cst[4 * st + 1], cm = cst[4 * st + 2];
             const int code = __float_as_int(cst[4 * st + 3].x);
             const uint32_t tile = s_tiles + st * a.tile_stride;
+            f32x2 t2[D / 2];
+#pragma unroll
+            for (int i = 0; i < D / 2; i++) t2[i] = 0ull;
+            switch (code) {                                           // uniform across the block
+                case 0: gather_tile<D, 2, 2, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t2); break;
+                case 1: gather_tile<D, 2, 3, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t2); break;
+                case 2: gather_tile<D, 3, 2, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t2); break;
+                default: gather_tile<D, 3, 3, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t2); break;
+            }
             float t[D];
 #pragma unroll
-            for (int i = 0; i < D; i++) t[i] = 0.f;
-            switch (code) {                                           // uniform across the block
-                case 0: gather_tile<D, 2, 2, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t); break;
-                case 1: gather_tile<D, 2, 3, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t); break;
-                case 2: gather_tile<D, 3, 2, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t); break;
-                default: gather_tile<D, 3, 3, SKIP>(cj, ck, cm, tile, pitch, bias, zeros, dxf, dyf, dzf, t); break;
-            }
+            for (int i = 0; i < D / 2; i++) unpack2(t2[i], t[2 * i], t[2 * i + 1]);
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_tile + 8 * st);          // this warp is done with the tile
             if (s >= 2) { mbar_wait(empty_a + 8 * sa, (uint32_t)(((s >> 1) - 1) & 1)); tc_fence_after(); }
@@ -358,7 +390,7 @@ template <int D, int NPAD>
 cudaError_t launch_brick(const CUtensorMap &tmap, const BrickArgs &a, cudaStream_t st)
 {
     using C = Cfg<D, NPAD>;
-    const size_t smem = (size_t)NST * a.tile_stride + (size_t)NST * C::BOP_BYTES + NST * 64 + 16 * NST + 48 + 16 + 64;
+    const size_t smem = (size_t)NST * a.tile_stride + (size_t)NST * C::BOP_BYTES + NST * 64 + 64 + 16 * NST + 48 + 16;
     // per launch: the attribute is per device, and this is cheaper than tracking which devices have it
     cudaError_t e = cudaFuncSetAttribute(adjoint_brick_kernel<D, NPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -395,12 +427,12 @@ int mm_adjoint_brick_launch(const mm_geometry *g, const AdjArgs &a, void *stream
     if (b.x_end <= b.x_begin) return cudaSuccess;
     b.nby = (a.Y + BY - 1) / BY; b.nbz = (a.Z + BZ - 1) / BZ;
     b.tj = g->brick_tj; b.tk = g->brick_tk;
-    b.tile_stride = (b.tj * b.tk * a.D * 4 + 127) & ~127;
+    b.tile_stride = (b.tj * b.tk * a.D * 4 + 1023) & ~1023;            // swizzled tiles: 1024-byte aligned stages
     b.bilinear = a.bilinear;
     alignas(64) CUtensorMap tmap;
     const unsigned long long n[4] = {(unsigned long long)a.D, (unsigned long long)a.Kd, (unsigned long long)a.J, (unsigned long long)a.P};
     const unsigned box[4] = {(unsigned)a.D, (unsigned)b.tk, (unsigned)b.tj, 1u};
-    if (!mm_tma_encode_4d_f32(&tmap, a.src, n, box)) return cudaErrorInvalidValue;
+    if (!mm_tma_encode_4d_f32(&tmap, a.src, n, box, a.D * 4)) return cudaErrorInvalidValue;
     const int NP = npad_for(a.ldk);
     float *bop = nullptr;
     cudaError_t e = mm_scratch_alloc((void **)&bop, (size_t)a.P * 2 * NP * a.D * sizeof(float), st);

@@ -517,12 +517,10 @@ cudaError_t launch_tc(const AdjArgs &a, cudaStream_t st)
     constexpr int KC = (D <= 16) ? 16 : D;
     constexpr int NPC = KC / D;
     const size_t smem = (size_t)4 * (TC_M * KC + NPAD * KC) * sizeof(float) + 4 * NPC * sizeof(TcProj) + 6 * sizeof(uint64_t) + 16;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(adjoint_tc_kernel<D, NPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // every launch: the attribute is per device (a process-wide "configured" flag breaks the second device) and the
+    // call costs a few hundred nanoseconds
+    const cudaError_t e = cudaFuncSetAttribute(adjoint_tc_kernel<D, NPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     const long long nvox = a.vox_end - a.vox_begin;
     if (nvox <= 0) return cudaSuccess;
     adjoint_tc_kernel<D, NPAD><<<(unsigned)((nvox + TC_M - 1) / TC_M), TC_THREADS, smem, st>>>(a);

@@ -63,6 +63,7 @@ struct mm_geometry {
 };
 
 void mm_set_error(const std::string &msg);
+void mm_note_launches(int n);          // kernels enqueued outside mm_kernels.cu (mm_launch_count accounting)
 
 // Arguments of the voxel-stationary (adjoint) kernels.
 struct AdjArgs {
@@ -82,7 +83,7 @@ cudaError_t mm_scratch_alloc(void **p, size_t bytes, cudaStream_t st);
 cudaError_t mm_scratch_free(void *p, cudaStream_t st);
 void mm_scratch_trim();
 bool mm_tma_available();
-bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long long n[4], const unsigned box[4]);
+bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long long n[4], const unsigned box[4], int swizzle);
 
 // mm_adjoint_brick.cu: fused adjoint, voxel bricks + TMA-staged detector tiles + tcgen05 (3xTF32), the primary path
 bool mm_adjoint_brick_supported(const mm_geometry *g, const AdjArgs &a);

@@ -22,6 +22,7 @@
 static std::atomic<long long> g_launches{0};
 
 extern "C" int64_t mm_launch_count(void) { return (int64_t)g_launches.load(); }
+void mm_note_launches(int n) { g_launches.fetch_add(n); }
 
 static thread_local cudaEvent_t g_phase_event = nullptr;
 
@@ -65,6 +66,7 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
 struct FwdArgs {
     const MMProj *tab;
     const float *vol;
+    int zero_vox;             // LERP only: vol is the library's copy [N+1][ldk] whose last record (index N) is all zeros
     int K, ldk;
     int X, Y, Z, J, Kd, P;
     float *proj;              // MODE 0 out [P][J][Kd][ldk]
@@ -131,6 +133,29 @@ __device__ __forceinline__ void ldg_nc_vec(const float *p, float (&v)[VEC])
     }
 }
 
+// Packed fp32 pairs (sm_100: add/sub/fma .f32x2 -> FADD2/FFMA2): two adjacent channels in one 64-bit register.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+// read-only 32- and 16-byte loads as pairs, in program order like ldg_nc_vec
+__device__ __forceinline__ void ldg_nc_pairs4(const float *p, f32x2 (&v)[4])
+{
+    asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v[0]), "=l"(v[1]), "=l"(v[2]), "=l"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void ldg_nc_pairs2(const float *p, f32x2 (&v)[2])
+{
+    asm volatile("ld.global.nc.v2.b64 {%0,%1}, [%2];" : "=l"(v[0]), "=l"(v[1]) : "l"(p));
+}
+// bilinear value of a pair of channels from its four taps as nested differences: c00 + fu (c10 - c00), ... (see LERP)
+__device__ __forceinline__ f32x2 lerp2(f32x2 c00, f32x2 c10, f32x2 c01, f32x2 c11, f32x2 fu, f32x2 fv)
+{
+    const f32x2 t0 = fma2(fu, sub2(c10, c00), c00), t1 = fma2(fu, sub2(c11, c01), c01);
+    return fma2(fv, sub2(t1, t0), t0);
+}
+
 // keep the slabs n in [lo,hi] on which -1 < A + n*s < N can hold (one slab of slack on each side)
 __device__ __forceinline__ void clip_range(double A, double s, int N, double &lo, double &hi)
 {
@@ -162,7 +187,7 @@ struct __align__(16) SlabTaps {
 // COOP (VEC == 4 only): the G lanes of a ray take turns at the index arithmetic — lane q works out the taps of
 // slab nb+q once, parks them in shared memory, and all lanes then stream through G slabs doing nothing but
 // loads and FMAs (v1 spent 21 instructions per LDG.128, profiles/r01_ncu_c5_v1.md).
-template <int VEC, int G, int NQ, int DMAX, int MODE, bool COOP>
+template <int VEC, int G, int NQ, int DMAX, int MODE, bool COOP, bool LERP = false>
 __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MINB8 : FWD_MINB) john_forward_kernel(const FwdArgs a)
 {
     constexpr int RPB = 256 / G;                  // rays per block
@@ -175,6 +200,14 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     // so a warp's request touches each 192-byte record in a 128-byte and a 64-byte piece: 2.5 cache lines per
     // tap on average against 3 for three 64-byte pieces (a load costs one L1 wavefront per distinct line).
     constexpr bool MIX = FWD_MIX48 && VEC == 4 && G == 4 && NQ == 3;
+    // LERP (MIX only; the volume is the library's own copy with an all-zero record appended): the bilinear value of a
+    // slab is formed as nested differences, c00 + fu (c10 - c00) etc., in packed fp32 pairs.  A constant (or slowly
+    // varying) field is then reproduced exactly, so a run of slabs through a uniform region adds exact multiples of
+    // the voxel value.  Four weighted FMAs make the partial sums of such a run approach powers of two from below,
+    // where round-to-nearest is one-sided: a bias of ~-0.2 ulp per slab, coherent over all rays and amplified by A^T
+    // (config 5's clipped-ellipsoid density: E_inf(grad) 9e-6 on its own data recipe, nine tenths of it this bias;
+    // 1.3e-6 with the nested form).  Taps outside the volume read the zero record, so no 0 x voxel product exists.
+    static_assert(!LERP || MIX, "LERP is the ldk = 48 path");
     auto chan = [&](int t) -> int {               // first channel of accumulator vector t of this lane
         if constexpr (MIX) return t < 2 ? 8 * q + 4 * t : 32 + 4 * q;
         else return VEC * (q + G * t);
@@ -213,7 +246,14 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     for (int t = 0; t < NQ; t++)
 #pragma unroll
         for (int x = 0; x < VEC; x++) { acc[t][x] = 0.f; tot[t][x] = 0.0; }
+    f32x2 acc2[LERP ? 6 : 1];                     // LERP: the same twelve round sums as packed pairs
+#pragma unroll
+    for (int i = 0; i < (LERP ? 6 : 1); i++) acc2[i] = 0ull;
     auto flush = [&]() {
+        if constexpr (LERP) {
+#pragma unroll
+            for (int i = 0; i < 6; i++) { unpack2(acc2[i], acc[i / 2][2 * (i % 2)], acc[i / 2][2 * (i % 2) + 1]); acc2[i] = 0ull; }
+        }
 #pragma unroll
         for (int t = 0; t < NQ; t++)
 #pragma unroll
@@ -247,6 +287,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         // tap offsets are counted in lane vectors (VEC floats)
         const int ldk4 = a.ldk / VEC;
         const int sM4 = (int)(sM / VEC), sU4 = (int)(sU / VEC), sV4 = (int)(sV / VEC);
+        const int zero_off = LERP ? a.zero_vox * ldk4 : 0;
         int rounds = (n1 >= n0) ? (n1 - n0 + G) / G : 0;
         rounds = __reduce_max_sync(0xffffffffu, rounds);          // the warp's groups step through rounds together
         for (int rd = 0; rd < rounds; rd++) {
@@ -267,10 +308,21 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                     const int b0 = n * sM4 + (u0 ? iu * sU4 : 0), b1 = n * sM4 + (u1 ? (iu + 1) * sU4 : 0);
                     const int c0 = v0 ? iv * sV4 : 0, c1 = v1 ? (iv + 1) * sV4 : 0;
                     t.o00 = b0 + c0; t.o10 = b1 + c0; t.o01 = b0 + c1; t.o11 = b1 + c1;
-                    t.w00 = (u0 && v0) ? (1.f - fu) * (1.f - fv) : 0.f;
-                    t.w10 = (u1 && v0) ? fu * (1.f - fv) : 0.f;
-                    t.w01 = (u0 && v1) ? (1.f - fu) * fv : 0.f;
-                    t.w11 = (u1 && v1) ? fu * fv : 0.f;
+                    if constexpr (LERP) {
+                        // taps outside the volume read the all-zero record (zero padding, S8); the table carries the fractions
+                        if (!(u0 && v0)) t.o00 = zero_off;
+                        if (!(u1 && v0)) t.o10 = zero_off;
+                        if (!(u0 && v1)) t.o01 = zero_off;
+                        if (!(u1 && v1)) t.o11 = zero_off;
+                        t.w00 = fu; t.w10 = fv;
+                    } else {
+                        t.w00 = (u0 && v0) ? (1.f - fu) * (1.f - fv) : 0.f;
+                        t.w10 = (u1 && v0) ? fu * (1.f - fv) : 0.f;
+                        t.w01 = (u0 && v1) ? (1.f - fu) * fv : 0.f;
+                        t.w11 = (u1 && v1) ? fu * fv : 0.f;
+                    }
+                } else if constexpr (LERP) {
+                    t.o00 = t.o10 = t.o01 = t.o11 = zero_off;
                 }
                 tap_o[r][q] = make_int4(t.o00, t.o10, t.o01, t.o11);
                 tap_w[r][q] = make_float4(t.w00, t.w10, t.w01, t.w11);
@@ -287,7 +339,41 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                     o[uu] = tap_o[r][i + uu];
                     w[uu] = tap_w[r][i + uu];
                 }
-                if constexpr (MIX) {
+                if constexpr (LERP) {
+                    const float *base = a.vol + 8 * q, *base2 = a.vol + 32 + 4 * q;
+#pragma unroll
+                    for (int hh = 0; hh < U; hh += 2) {           // 32-byte pieces, two slabs at a time
+                        f32x2 c[2][4][4];
+#pragma unroll
+                        for (int uu = 0; uu < 2; uu++) {
+                            ldg_nc_pairs4(base + (long long)o[hh + uu].x * 4, c[uu][0]);
+                            ldg_nc_pairs4(base + (long long)o[hh + uu].y * 4, c[uu][1]);
+                            ldg_nc_pairs4(base + (long long)o[hh + uu].z * 4, c[uu][2]);
+                            ldg_nc_pairs4(base + (long long)o[hh + uu].w * 4, c[uu][3]);
+                        }
+                        if (hh == 0) flush();                     // the previous step's sums, under this step's load latency
+#pragma unroll
+                        for (int uu = 0; uu < 2; uu++) {
+                            const f32x2 fu = pack2(w[hh + uu].x, w[hh + uu].x), fv = pack2(w[hh + uu].y, w[hh + uu].y);
+#pragma unroll
+                            for (int x = 0; x < 4; x++) acc2[x] = add2(acc2[x], lerp2(c[uu][0][x], c[uu][1][x], c[uu][2][x], c[uu][3][x], fu, fv));
+                        }
+                    }
+                    f32x2 c[U][4][2];                             // 16-byte pieces
+#pragma unroll
+                    for (int uu = 0; uu < U; uu++) {
+                        ldg_nc_pairs2(base2 + (long long)o[uu].x * 4, c[uu][0]);
+                        ldg_nc_pairs2(base2 + (long long)o[uu].y * 4, c[uu][1]);
+                        ldg_nc_pairs2(base2 + (long long)o[uu].z * 4, c[uu][2]);
+                        ldg_nc_pairs2(base2 + (long long)o[uu].w * 4, c[uu][3]);
+                    }
+#pragma unroll
+                    for (int uu = 0; uu < U; uu++) {
+                        const f32x2 fu = pack2(w[uu].x, w[uu].x), fv = pack2(w[uu].y, w[uu].y);
+#pragma unroll
+                        for (int x = 0; x < 2; x++) acc2[4 + x] = add2(acc2[4 + x], lerp2(c[uu][0][x], c[uu][1][x], c[uu][2][x], c[uu][3][x], fu, fv));
+                    }
+                } else if constexpr (MIX) {
                     const float *base = a.vol + 8 * q, *base2 = a.vol + 32 + 4 * q;
 #pragma unroll
                     for (int h = 0; h < U; h += 2) {              // 32-byte pieces, two slabs at a time
@@ -739,7 +825,7 @@ __global__ void laplacian_kernel(const float *__restrict__ in, float *__restrict
 //   M_xx = c_0/3 - c_3/(3 sqrt5) + c_5/sqrt15, M_yy = c_0/3 - c_3/(3 sqrt5) - c_5/sqrt15, M_zz = c_0/3 + 2 c_3/(3 sqrt5).
 // Eigenvalues of the symmetric 3x3 by the trigonometric formula, eigenvectors from cross products of the rows of
 // M - lambda I; all in fp64 (a few hundred flops per voxel against 24..192 bytes of traffic).
-__device__ __forceinline__ void eigvec3(const double M[6], double lam, double v[3])
+__device__ __forceinline__ void eigvec3(const double M[6], double lam, double v[3], double *quality)
 {
     // rows of A = M - lam I; the eigenvector is orthogonal to all of them: take the largest cross product
     const double r0[3] = {M[0] - lam, M[3], M[4]}, r1[3] = {M[3], M[1] - lam, M[5]}, r2[3] = {M[4], M[5], M[2] - lam};
@@ -752,8 +838,47 @@ __device__ __forceinline__ void eigvec3(const double M[6], double lam, double v[
         const double n = c[i][0] * c[i][0] + c[i][1] * c[i][1] + c[i][2] * c[i][2];
         if (n > bn) { bn = n; best = i; }
     }
+    *quality = bn;                                                       // ~ (gap to the other eigenvalues)^4: 0 when lam is repeated
     if (bn > 0.0) { const double s = rsqrt(bn); v[0] = c[best][0] * s; v[1] = c[best][1] * s; v[2] = c[best][2] * s; }
-    else { v[0] = 1.0; v[1] = 0.0; v[2] = 0.0; }                      // degenerate (isotropic): any unit vector
+    else { v[0] = 1.0; v[1] = 0.0; v[2] = 0.0; }
+}
+
+// Orthonormal eigenvectors of the symmetric M for eigenvalues l[0] >= l[1] >= l[2].  The vector of the best-isolated
+// eigenvalue comes from eigvec3; when two eigenvalues (nearly) coincide the other two are ANY orthonormal pair of the
+// orthogonal plane (a valid eigenbasis of the repeated eigenvalue), completed by Gram-Schmidt; M = lambda I gives the
+// identity frame.  `tiny` = the scale below which a gap counts as zero.
+__device__ __forceinline__ void eigframe3(const double M[6], const double l[3], double tiny, double V[3][3])
+{
+    const double g01 = l[0] - l[1], g12 = l[1] - l[2];
+    if (g01 <= tiny && g12 <= tiny) {                                    // isotropic
+        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) V[i][j] = i == j ? 1.0 : 0.0;
+        return;
+    }
+    double q;
+    const int iso = g01 >= g12 ? 0 : 2;                                  // the eigenvalue farthest from the other two
+    eigvec3(M, l[iso], V[iso], &q);
+    const int other = 2 - iso;                                           // 2 or 0; the middle one is index 1
+    double qo;
+    eigvec3(M, l[other], V[other], &qo);
+    const double gap_mid = iso == 0 ? g12 : g01;
+    // project the isolated vector out and renormalise; fall back to a coordinate axis in the plane when the pair is repeated
+    double d = V[other][0] * V[iso][0] + V[other][1] * V[iso][1] + V[other][2] * V[iso][2];
+    double w[3] = {V[other][0] - d * V[iso][0], V[other][1] - d * V[iso][1], V[other][2] - d * V[iso][2]};
+    double n = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+    if (gap_mid <= tiny || n < 0.25) {
+        // repeated pair: any unit vector orthogonal to V[iso]; start from the coordinate axis least aligned with it
+        const double ax = fabs(V[iso][0]), ay = fabs(V[iso][1]), az = fabs(V[iso][2]);
+        double e[3] = {0.0, 0.0, 0.0};
+        e[(ax <= ay && ax <= az) ? 0 : (ay <= az ? 1 : 2)] = 1.0;
+        d = e[0] * V[iso][0] + e[1] * V[iso][1] + e[2] * V[iso][2];
+        w[0] = e[0] - d * V[iso][0]; w[1] = e[1] - d * V[iso][1]; w[2] = e[2] - d * V[iso][2];
+        n = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+    }
+    const double s = rsqrt(n);
+    V[other][0] = w[0] * s; V[other][1] = w[1] * s; V[other][2] = w[2] * s;
+    // the middle vector completes the right-handed frame: iso x other (or other x iso)
+    const double *a = V[iso], *b = V[other];
+    V[1][0] = a[1] * b[2] - a[2] * b[1]; V[1][1] = a[2] * b[0] - a[0] * b[2]; V[1][2] = a[0] * b[1] - a[1] * b[0];
 }
 
 __global__ void derived_kernel(const float *__restrict__ vol, int ldk, int K, long long nvox, float *__restrict__ mean,
@@ -785,10 +910,10 @@ __global__ void derived_kernel(const float *__restrict__ vol, int ldk, int K, lo
     if (moments) { for (int i = 0; i < 6; i++) moments[vox * 6 + i] = (float)M[i]; }   // xx, yy, zz, xy, xz, yz  (Eq. 11)
     if (eig) { eig[vox * 3] = (float)l[0]; eig[vox * 3 + 1] = (float)l[1]; eig[vox * 3 + 2] = (float)l[2]; }
     if (vec) {
+        double V[3][3];
+        eigframe3(M, l, 1e-12 * fmax(fabs(l[0]), fabs(l[2])), V);
         for (int i = 0; i < 3; i++) {
-            double v[3];
-            eigvec3(M, l[i], v);
-            vec[vox * 9 + 3 * i] = (float)v[0]; vec[vox * 9 + 3 * i + 1] = (float)v[1]; vec[vox * 9 + 3 * i + 2] = (float)v[2];
+            vec[vox * 9 + 3 * i] = (float)V[i][0]; vec[vox * 9 + 3 * i + 1] = (float)V[i][1]; vec[vox * 9 + 3 * i + 2] = (float)V[i][2];
         }
     }
     if (fa) {                                                           // Eq. 12
@@ -900,7 +1025,14 @@ mm_status check_common(const mm_geometry *g, int K, int ldk, const char *who)
     if (!g) { mm_set_error(std::string(who) + ": NULL geometry"); return MM_ERR_NULL; }
     if (!g->d_table) { mm_set_error(std::string(who) + ": geometry was created without a CUDA device (no CPU fallback)"); return MM_ERR_CUDA; }
     if (K < 1 || ldk < K) { mm_set_error(std::string(who) + ": need 1 <= K <= ldk"); return MM_ERR_SHAPE; }
-    if (K > 256) { mm_set_error(std::string(who) + ": K > 256 is not supported"); return MM_ERR_UNSUPPORTED; }
+    if (K > 256 || ldk > 256) { mm_set_error(std::string(who) + ": K, ldk > 256 are not supported"); return MM_ERR_UNSUPPORTED; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != g->device) {
+        cudaGetLastError();
+        mm_set_error(std::string(who) + ": the geometry was created on CUDA device " + std::to_string(g->device) +
+                     ", the current device is " + std::to_string(dev));
+        return MM_ERR_VALUE;
+    }
     return MM_OK;
 }
 
@@ -921,9 +1053,38 @@ void launch_fwd(const FwdArgs &a, cudaStream_t st)
     john_forward_kernel<VEC, G, NQ, DMAX, MODE, false><<<(unsigned)tiles, 256, 0, st>>>(a);
 }
 
+// ldk = 48 (K = 45, configs 3 and 5): march a copy of the volume with an all-zero record appended (stream-ordered
+// scratch from the library's pool; the copy costs 2 x 3.2 GB of traffic on config 5, ~1 ms before a 175 ms march) in
+// the nested-difference form (LERP).  Returns false if the scratch could not be had; the caller then takes the
+// weighted-FMA path on the caller's own buffer.
+template <int DMAX, int MODE>
+bool launch_fwd_lerp(const FwdArgs &a, cudaStream_t st)
+{
+    const long long nvox = (long long)a.X * a.Y * a.Z;
+    if ((nvox + 1) * 12 >= (1LL << 31)) return false;           // tap offsets are 32-bit float4 indices
+    float *scratch = nullptr;
+    if (mm_scratch_alloc((void **)&scratch, (size_t)(nvox + 1) * 48 * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return false; }
+    bool ok = cudaMemcpyAsync(scratch, a.vol, (size_t)nvox * 48 * sizeof(float), cudaMemcpyDeviceToDevice, st) == cudaSuccess &&
+              cudaMemsetAsync(scratch + nvox * 48, 0, 48 * sizeof(float), st) == cudaSuccess;
+    if (ok) {
+        FwdArgs b = a;
+        b.vol = scratch; b.zero_vox = (int)nvox;
+        constexpr int TK = 8, TJ = 8;                           // 64 rays per block (G = 4)
+        const long long tiles = (long long)a.P * ((a.J + TJ - 1) / TJ) * ((a.Kd + TK - 1) / TK);
+        john_forward_kernel<4, 4, 3, DMAX, MODE, true, true><<<(unsigned)tiles, 256, 0, st>>>(b);
+    } else {
+        cudaGetLastError();
+    }
+    mm_scratch_free(scratch, st);
+    return ok;
+}
+
 template <int DMAX, int MODE>
 mm_status dispatch_fwd(const FwdArgs &a, bool vec, cudaStream_t st)
 {
+    static const bool lerp_off = getenv("MM_DISABLE_LERP") != nullptr;     // debugging switch: weighted FMAs on the caller's buffer
+    if (vec && a.ldk == 48 && !lerp_off && launch_fwd_lerp<DMAX, MODE>(a, st))
+        return check_launch("john_forward_kernel (nested-difference form)");
     // 48 floats per voxel (K = 45, configs 3 and 5) = 12 float4 = 4 lanes x 3: every lane's load is used.  The
     // 8 x 32-byte layout below would idle 2 lanes in 8, and the register write-back of a load costs the same
     // 8 wavefronts whether or not its lanes carry new data (profiles/r01_ncu_c5_v5.md): 198 -> 191 ms on config 5.
@@ -963,7 +1124,7 @@ mm_status dispatch_fwd_d(const FwdArgs &a, bool vec, cudaStream_t st)
 
 void fill_fwd(FwdArgs &a, const mm_geometry *g, const float *vol, int K, int ldk)
 {
-    a.tab = g->d_table; a.vol = vol; a.K = K; a.ldk = ldk;
+    a.tab = g->d_table; a.vol = vol; a.zero_vox = 0; a.K = K; a.ldk = ldk;
     a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
     a.proj = nullptr; a.B = nullptr; a.D = 0; a.data = nullptr; a.weights = nullptr; a.sino = nullptr; a.loss = nullptr;
     a.huber = 0.f;

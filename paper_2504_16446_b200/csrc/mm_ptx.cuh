@@ -36,6 +36,20 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
+// same, but the hardware may keep the thread suspended for up to `ns` nanoseconds waiting for the phase (it wakes at
+// once when the phase completes): a polling warp then costs (almost) no issue slots
+__device__ __forceinline__ bool mbar_try_wait_suspend(uint32_t bar, uint32_t parity, uint32_t ns)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity), "r"(ns)
+        : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ uint64_t globaltimer_ns()
 {
     uint64_t t;
@@ -49,8 +63,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     if (mbar_try_wait(bar, parity)) return;
     const uint64_t t0 = globaltimer_ns();
-    while (!mbar_try_wait(bar, parity))
-        if (globaltimer_ns() - t0 > 20000000000ull) __trap();
+    for (uint32_t polls = 1; !mbar_try_wait_suspend(bar, parity, 100000u); polls++)
+        if ((polls & 63u) == 0 && globaltimer_ns() - t0 > 20000000000ull) __trap();
 }
 
 // ---- TMA ----------------------------------------------------------------------------------------------------
@@ -144,9 +158,11 @@ __device__ __forceinline__ void tc_commit(uint32_t bar)
 
 // x = hi + lo: hi = x rounded to nearest TF32 (1+8+10 bits), lo = x - hi exactly (|lo| <= 2^-11 |x|, either sign).
 // The tensor core ignores the 13 low mantissa bits of lo (error <= 2^-21 |x|, unbiased because lo's sign is random).
+// (cvt.rna.tf32.f32 compiles to add, NaN/Inf test, select, mask; finite data needs only the add and the mask:
+// round-half-away on the magnitude bits is exactly rna.)
 __device__ __forceinline__ void split_tf32(float x, uint32_t &hi, uint32_t &lo)
 {
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
+    hi = (__float_as_uint(x) + 0x1000u) & 0xffffe000u;
     lo = __float_as_uint(x - __uint_as_float(hi));
 }
 

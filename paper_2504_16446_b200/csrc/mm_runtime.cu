@@ -3,6 +3,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <stdlib.h>
+
 #include <mutex>
 #include <string>
 
@@ -62,15 +64,25 @@ EncodeTiledFn encode_tiled_fn()
 
 }  // namespace
 
+// MM_SCRATCH_MALLOC=1 (debugging/profiling only: ncu's kernel replay cannot save and restore pool memory): plain
+// cudaMalloc / cudaFree, which synchronise.
+static bool scratch_plain() { static const bool v = getenv("MM_SCRATCH_MALLOC") != nullptr; return v; }
+
 cudaError_t mm_scratch_alloc(void **p, size_t bytes, cudaStream_t st)
 {
+    if (scratch_plain()) return cudaMalloc(p, bytes ? bytes : 16);
     cudaMemPool_t pool;
     cudaError_t e = pool_for_current_device(&pool);
     if (e != cudaSuccess) return e;
     return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st);
 }
 
-cudaError_t mm_scratch_free(void *p, cudaStream_t st) { return p ? cudaFreeAsync(p, st) : cudaSuccess; }
+cudaError_t mm_scratch_free(void *p, cudaStream_t st)
+{
+    if (!p) return cudaSuccess;
+    if (scratch_plain()) { cudaStreamSynchronize(st); return cudaFree(p); }
+    return cudaFreeAsync(p, st);
+}
 
 void mm_scratch_trim()
 {
@@ -81,8 +93,10 @@ void mm_scratch_trim()
 
 bool mm_tma_available() { return encode_tiled_fn() != nullptr; }
 
-// fp32 tensor [n3][n2][n1][n0] (n0 innermost, dense), box [1][b2][b1][b0]; out-of-bounds reads give 0
-bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long long n[4], const unsigned b[4])
+// fp32 tensor [n3][n2][n1][n0] (n0 innermost, dense), box [b3][b2][b1][b0]; out-of-bounds reads give 0.  swizzle = 0, 32,
+// 64 or 128 bytes: the box lands in shared memory with that swizzle (the low log2(swizzle/16) bits of the 16-byte chunk
+// index are XORed with the same number of bits of the 128-byte row index); swizzle must equal b0 * 4 here.
+bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long long n[4], const unsigned b[4], int swizzle)
 {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
@@ -91,7 +105,10 @@ bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long 
     cuuint32_t box[4] = {b[0], b[1], b[2], b[3]};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = fn((CUtensorMap *)tmap_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void *>(base), dims, strides, box,
-                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                         : swizzle == 32 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         mm_set_error("cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r));

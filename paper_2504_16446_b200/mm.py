@@ -13,13 +13,13 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmm.so")
+LIB_PATH = os.environ.get("MM_LIB_PATH") or os.path.join(_HERE, "libmm.so")     # MM_LIB_PATH: an alternative build (kernel experiments)
 _lib = None
 
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
-           "mm_axpy_precond", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
+           "mm_axpy_precond", "mm_iterate", "mm_workspace_release", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -35,6 +35,11 @@ class _Desc(ctypes.Structure):
                 ("q0_dir", ctypes.c_double * 3), ("q90_dir", ctypes.c_double * 3),
                 ("inner_axis", ctypes.c_double * 3), ("outer_axis", ctypes.c_double * 3),
                 ("voxel_size", ctypes.c_double), ("pixel_size", ctypes.c_double)]
+
+
+class _IterParams(ctypes.Structure):
+    _fields_ = [("eta", ctypes.c_float), ("momentum", ctypes.c_float), ("mu_laplacian", ctypes.c_float), ("mu_l2", ctypes.c_float),
+                ("max_iter", ctypes.c_int32), ("check_every", ctypes.c_int32), ("tol", ctypes.c_double)]
 
 
 def load():
@@ -73,6 +78,8 @@ def load():
     L.mm_axpy_precond.argtypes = [vp, vp, vp, ctypes.c_float, i64, vp]
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
     L.mm_host_workspace_release.argtypes = []
+    L.mm_workspace_release.argtypes = []
+    L.mm_iterate.argtypes = [vp, vp, i32, i32, i32, vp, vp, ctypes.POINTER(_IterParams), vp, vp, vp, ctypes.POINTER(i32), vp]
     L.mm_set_phase_event.argtypes = [vp]
     L.mm_launch_count.restype = i64
     L.mm_launch_count.argtypes = []
@@ -334,6 +341,25 @@ def mm_nesterov_step(c, v, grad, eta: float, momentum: float, stream=None):
     _check(load().mm_nesterov_step(_dev(c, c.shape, "c"), _dev(v, c.shape, "v"), _dev(grad, c.shape, "grad"), float(eta),
                                    float(momentum), c.numel(), _stream(stream)), "mm_nesterov_step")
     return c, v
+
+
+def mm_iterate(g: Geometry, B, K: int, data, weights, c, v, losses, eta: float, momentum: float = 0.0, mu_laplacian: float = 0.0,
+               mu_l2: float = 0.0, max_iter: int = 20, tol: float = 0.0, check_every: int = 1, stream=None) -> int:
+    """device-resident regularised Nesterov iteration; c, v in/out, losses: CUDA float64 [max_iter]; returns n_iter."""
+    import torch
+    ldk, D = c.shape[-1], B.shape[-1]
+    w = ctypes.c_void_p(None) if weights is None else _dev(weights, g.proj_shape(D), "weights")
+    p = _IterParams(float(eta), float(momentum), float(mu_laplacian), float(mu_l2), int(max_iter), int(check_every), float(tol))
+    n = ctypes.c_int32(0)
+    _check(load().mm_iterate(g._h, _dev(B, (g.P, K, D), "B"), K, ldk, D, _dev(data, g.proj_shape(D), "data"), w, ctypes.byref(p),
+                             _dev(c, g.vol_shape(ldk), "c"), _dev(v, g.vol_shape(ldk), "v"),
+                             _dev(losses, (int(max_iter),), "losses", torch.float64), ctypes.byref(n), _stream(stream)), "mm_iterate")
+    return n.value
+
+
+def mm_workspace_release():
+    """Return the library's cached device memory (host-call arena and stream-ordered scratch pool) to the driver."""
+    _check(load().mm_workspace_release(), "mm_workspace_release")
 
 
 def mm_axpy(c, grad, eta: float, stream=None):

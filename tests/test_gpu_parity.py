@@ -273,6 +273,19 @@ def test_gpu_dot_product_identity(mm):
     mm.mm_adjoint(gm, B, ys, K, ATy)
     lhs, rhs = (Axs.double() * ys.double()).sum().item(), (x.double() * ATy.double()).sum().item()
     assert abs(lhs - rhs) <= 1e-5 * (Axs.double().norm() * ys.double().norm()).item(), (lhs, rhs)
+    # non-cancelling case: x, y >= 0 (and the John transform has non-negative entries), so <Ax,y> is a sum of
+    # non-negative terms and the identity must hold to 1e-5 of the inner product itself
+    xp, yp = x.abs(), y.abs()
+    mm.mm_john_forward(gm, xp, K, Ax)
+    mm.mm_john_adjoint(gm, yp, K, ATy)
+    lhs, rhs = (Ax.double() * yp.double()).sum().item(), (xp.double() * ATy.double()).sum().item()
+    assert lhs > 0 and abs(lhs - rhs) <= 1e-5 * lhs, (lhs, rhs)
+    # same through the fused pair with |B| (A = P (x) |B| is then non-negative too)
+    absB = B.abs()
+    mm.mm_forward(gm, absB, xp, K, Axs)
+    mm.mm_adjoint(gm, absB, ys.abs(), K, ATy)
+    lhs, rhs = (Axs.double() * ys.abs().double()).sum().item(), (xp.double() * ATy.double()).sum().item()
+    assert lhs > 0 and abs(lhs - rhs) <= 1e-5 * lhs, (lhs, rhs)
 
 
 def test_zero_residual_and_zero_weight(mm):
@@ -602,6 +615,12 @@ def test_derived_quantities(ora, mm, name, shape):
     vol[..., K:] = 7.0                                                 # pad channels must be ignored
     vol[0, 0, 0, :K] = 0.0                                             # an empty voxel: M = 0, FA = 0
     vol[1, 1, 1, :K] = 0.0; vol[1, 1, 1, 0] = 2.0                      # an isotropic voxel: degenerate eigenvalues
+    # an exactly fibre-symmetric voxel about an oblique axis n: c_2m = Y_2m(n) (closed forms, 4pi-normalised) gives
+    # M = a I + b n n^T, a repeated eigenvalue whose plane contains no coordinate axis
+    nx, ny, nz = 0.48, -0.6, 0.64
+    s15, s5 = math.sqrt(15.0), math.sqrt(5.0)
+    vol[2, 2, 2, :K] = 0.0; vol[2, 2, 2, 0] = 1.0
+    vol[2, 2, 2, 1:6] = [s15 * nx * ny, s15 * ny * nz, 0.5 * s5 * (3 * nz * nz - 1), s15 * nx * nz, 0.5 * s15 * (nx * nx - ny * ny)]
     gm = mm.Geometry(cfg.shape, cfg.det, [0.0], [0.0])
     mean = torch.empty(cfg.shape, device="cuda"); fa = torch.empty(cfg.shape, device="cuda")
     mom = torch.empty(cfg.shape + (6,), device="cuda"); eig = torch.empty(cfg.shape + (3,), device="cuda")
@@ -618,6 +637,9 @@ def test_derived_quantities(ora, mm, name, shape):
     assert np.abs(e - d["eig"]).max() <= TOL * scale
     v = vec.cpu().numpy().astype(np.float64)
     assert np.abs(np.linalg.norm(v, axis=-1) - 1.0).max() < 1e-5
+    gram = np.einsum("...ij,...kj->...ik", v, v)
+    assert np.abs(gram - np.eye(3)).max() < 1e-5                          # an orthonormal frame at every voxel, degenerate or not
+    assert np.abs(np.abs(v[2, 2, 2] @ np.array([nx, ny, nz])) - np.array([1.0, 0.0, 0.0])).max() < 1e-5   # fibre axis first, the rest orthogonal
     resid = np.einsum("...ij,...kj->...ki", d["M"], v) - d["eig"][..., :, None] * v
     assert np.abs(resid).max() <= 1e-4 * scale                          # valid eigenvectors everywhere
     g01, g12 = np.abs(d["eig"][..., 0] - d["eig"][..., 1]), np.abs(d["eig"][..., 1] - d["eig"][..., 2])
@@ -648,3 +670,51 @@ def test_l1_huber_tv_regularisers(ora, mm, K, ldk, shape):
         got = grad.cpu().numpy()
         assert abs(val.item() - R) <= 1e-5 * R
         assert np.abs(got[..., :K] - g_o).max() <= 2e-5 * max(1.0, np.abs(g_o).max()) and np.all(got[..., K:] == 0.0)
+
+
+@pytest.mark.parametrize("momentum,mu_lap,mu_l2,check_every", [(0.0, 0.0, 0.0, 1), (0.7, 1e-3, 1e-4, 1), (0.5, 0.0, 2e-4, 3)])
+def test_device_resident_iteration_with_stop_rule(ora, mm, momentum, mu_lap, mu_l2, check_every):
+    """NEXT-3: mm_iterate = the whole regularised Nesterov loop on the device with the relative-change stop rule
+    (reading S25) against the oracle's `iterate`: same stop iteration, same loss history,
+    same iterate; pad channels untouched; nothing but a 4-byte flag crosses the bus inside the loop."""
+    import torch
+    cfg, c = cfg_case("C2", (18, 16, 20), (22, 21), 3, seed=61, weights="mask")
+    go, gm = c.geoms(ora, mm)
+    K, ldk, D = c.K, c.ldk, c.D
+    B = mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(D))
+    data = synth.poisson_data(ora.forward(go, B, c.vol[..., :K]), cfg.counts, cfg.seed)
+    absB = np.abs(B)
+    lip = float(ora.forward(go, absB, np.ones(c.shape + (K,), np.float32)).max() *
+                ora.adjoint(go, absB, np.ones((c.P,) + c.det + (D,)), form="scatter").max())
+    mu_lap, mu_l2 = mu_lap * lip, mu_l2 * lip
+    eta = 1.0 / (lip + 144.0 * mu_lap + mu_l2)
+    max_iter = 30
+    start = np.zeros(c.shape + (K,), np.float32)
+    # tolerance placed between two consecutive relative changes of the (oracle) loss history, so that the rule must fire
+    # at a known check well inside the budget and no fp32-vs-fp64 difference can flip the decision
+    _, _, L_all = ora.iterate(go, B, data, c.w, start, eta, momentum, mu_lap, mu_l2, max_iter, 0.0)
+    rel = [abs(a - b) / b for a, b in zip(L_all[:-1], L_all[1:])]         # rel[k-1] is what the check after iteration k sees
+    k_stop = next(k for k in range(12, max_iter) if (k + 1) % check_every == 0)
+    tol = math.sqrt(rel[k_stop - 1] * rel[k_stop - 2])
+    assert rel[k_stop - 1] < 0.99 * tol and all(r > 1.01 * tol for r in rel[:k_stop - 1])
+    c_o, v_o, L_o = ora.iterate(go, B, data, c.w, start, eta, momentum, mu_lap, mu_l2, max_iter, tol, check_every=check_every)
+    assert len(L_o) == k_stop + 1
+    x = torch.zeros(gm.vol_shape(ldk), device="cuda"); v = torch.zeros_like(x)
+    x[..., K:] = 7.0                                                      # pad channels: ignored and left alone
+    losses = torch.full((max_iter,), float("nan"), device="cuda", dtype=torch.float64)
+    n0 = mm.mm_launch_count()
+    n = mm.mm_iterate(gm, dev(B), K, dev(data), dev(c.w), x, v, losses, eta, momentum, mu_lap, mu_l2, max_iter, tol, check_every)
+    torch.cuda.synchronize()
+    assert n == len(L_o)
+    got = losses.cpu().numpy()
+    assert np.all(np.isnan(got[n:])) and np.abs(got[:n] - np.array(L_o)).max() <= TOL_LOSS * max(L_o)
+    assert einf(x.cpu().numpy()[..., :K], c_o) <= 1e-4 and einf(v.cpu().numpy()[..., :K], v_o) <= 1e-4
+    assert torch.all(x[..., K:] == 7.0).item() and torch.all(v[..., K:] == 0.0).item()
+    assert mm.mm_launch_count() - n0 >= 5 * n                            # kernels ran; the loop is the library's
+    # tol <= 0: runs max_iter iterations without a single synchronisation
+    x2 = torch.zeros_like(x); v2 = torch.zeros_like(x)
+    l6 = torch.full((6,), float("nan"), device="cuda", dtype=torch.float64)
+    assert mm.mm_iterate(gm, dev(B), K, dev(data), dev(c.w), x2, v2, l6, eta, momentum, mu_lap, mu_l2, 6, 0.0, 1) == 6
+    _, _, L6 = ora.iterate(go, B, data, c.w, np.zeros(c.shape + (K,), np.float32), eta, momentum, mu_lap, mu_l2, 6, 0.0)
+    torch.cuda.synchronize()
+    assert np.abs(l6.cpu().numpy() - np.array(L6)).max() <= TOL_LOSS * max(L6)
