@@ -424,6 +424,57 @@ def ours(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def sparse_extra(args):
+    """`--sparse-extra`: NEXT-2 measurement (not the headline step).  Table V's largest basis (N = 162 directions, NN
+    indicator functions) on a 100^3 volume, 240 projections (6 tilts x 40), 100^2 detector, D = 8:
+    dense fused forward / gradient against the sparse-plan calls on the same NN matrix."""
+    import torch
+    from paper_2504_16446_b200 import mm
+    torch.cuda.set_device(0)
+    mm.load()
+    cfg = synth.get_config("C3", tilts_deg=(0.0, 9.0, 18.0, 27.0, 36.0, 45.0))
+    K, D = 162, 8
+    ldk = synth.ldk_for(K)
+    rot, tilt = synth.angles(cfg)
+    g = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
+    h_B = mm.mm_basis_grid_matrix(g, mm.MM_BASIS_NN, synth.grid_directions(K), *synth.segments(D), n_quad=8)
+    plan = mm.SparsePlan(g, h_B)
+    rng = np.random.default_rng(162)
+    vol = torch.from_numpy(synth.pad_channels(rng.uniform(0, 1, cfg.shape + (K,)).astype(np.float32), ldk)).cuda()
+    B = torch.from_numpy(h_B).cuda()
+    sino = torch.empty(g.proj_shape(D), device="cuda")
+    mm.mm_forward(g, B, vol, K, sino)
+    data = sino * (1 + 0.03 * torch.randn_like(sino))
+    grad = torch.empty(g.vol_shape(ldk), device="cuda")
+    wr = torch.empty_like(sino)
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+
+    def timed(fn):
+        for _ in range(max(3, args.warmup)):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    res = {"forward_dense_ms": timed(lambda: mm.mm_forward(g, B, vol, K, sino)),
+           "forward_sparse_ms": timed(lambda: mm.mm_forward_sparse(g, plan, B, vol, K, sino)),
+           "gradient_dense_ms": timed(lambda: mm.mm_loss_gradient(g, B, vol, K, data, None, grad, loss, wr)),
+           "gradient_sparse_ms": timed(lambda: mm.mm_loss_gradient_sparse(g, plan, B, vol, K, data, None, grad, loss, wr)),
+           "adjoint_dense_ms": timed(lambda: mm.mm_adjoint(g, B, wr, K, grad))}
+    line = {"what": "NEXT-2 sparse reciprocal-space map vs dense, NN basis (PAPER.md:242, 274)", "data": "synthetic",
+            "config": {"workload": f"100x100x100 voxels, K={K} NN directions (ldk {ldk}), P={g.P}, detector 100x100, D={D}, n_quad=8",
+                       "active_channels_per_projection": {"max": plan.max_active, "mean": plan.mean_active}},
+            "steps": args.steps, **res,
+            "forward_speedup": res["forward_dense_ms"] / res["forward_sparse_ms"],
+            "gradient_speedup": res["gradient_dense_ms"] / res["gradient_sparse_ms"]}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -433,12 +484,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true", help="also time mm_backproject (outside the step)")
+    ap.add_argument("--sparse-extra", action="store_true", help="time the NEXT-2 sparse-plan calls against the dense ones (K = 162 NN basis) and exit")
     ap.add_argument("--record-traffic", metavar="NCU_RAW_CSV", help="store the kernels' DRAM bytes from an ncu raw-page csv and exit")
     ap.add_argument("--traffic-command", default="ncu --set full --clock-control none -k regex:john_forward|adjoint_brick ... python bench.py --steps 1 --warmup 3 --no-cpu-baseline; ncu -i <rep> --page raw --csv")
     args = ap.parse_args()
     cfg = synth.get_config(args.config)
     if args.record_traffic:
         record_traffic(args.record_traffic, cfg.name, args.traffic_command)
+        return
+    if args.sparse_extra:
+        sparse_extra(args)
         return
     if args.impl == "reference":
         reference_arm(args, cfg)

@@ -199,6 +199,31 @@ mm_status mm_axpy_precond(float *c, const float *grad, const float *pre, float e
 mm_status mm_derived_quantities(const mm_geometry *g, const float *vol, int32_t K, int32_t ldk, float *mean, float *moments,
                                 float *eigenvalues, float *eigenvectors, float *fa, void *stream);
 
+/* NEXT-2 — sparse reciprocal-space map (the sparse pipelines "use a modified version of the John transform that
+ * calculates the reciprocal-space and real-space projection operations simultaneously within one kernel, using a
+ * sparse approximation to the reciprocal-space mapping ... such as only mapping one basis function to each segment").
+ * Reading S26: the approximation keeps, for every projection s and segment c, the n_keep coefficients B[s][i][c] of
+ * largest magnitude (lowest i first among equals) and zeroes the others.
+ *   mm_basis_sparsify       HOST: h_B [P][K][D] -> h_B_out (same shape; may not alias h_B); n_keep >= K copies.
+ *   mm_sparse_plan_create   HOST h_B (already sparse: an NN basis, or the output of mm_basis_sparsify): records for every
+ *                           projection the channels i with a non-zero row B[s][i][:] and uploads the lists.  The plan
+ *                           belongs to (g, K, D) and must be rebuilt when the zero pattern of B changes.
+ *   mm_sparse_plan_info     max / mean number of active channels per projection; counts [P] HOST or NULL.
+ *   mm_forward_sparse       = mm_forward with that B, marching only the active channels of each projection.
+ *   mm_loss_gradient_sparse = mm_loss_gradient with that B: sparse phase 1, dense tensor-core contraction in phase 2.
+ * B (DEVICE) must have the zero pattern the plan was made from: rows outside the lists are never read.  Results equal
+ * the dense calls' on the same B to fp32 rounding. */
+typedef struct mm_sparse_plan mm_sparse_plan;
+mm_status mm_basis_sparsify(const float *h_B, int32_t P, int32_t K, int32_t D, int32_t n_keep, float *h_B_out);
+mm_status mm_sparse_plan_create(const mm_geometry *g, const float *h_B, int32_t K, int32_t D, mm_sparse_plan **out);
+mm_status mm_sparse_plan_destroy(mm_sparse_plan *plan);
+mm_status mm_sparse_plan_info(const mm_sparse_plan *plan, int32_t *max_active, double *mean_active, int32_t *counts);
+mm_status mm_forward_sparse(const mm_geometry *g, const mm_sparse_plan *plan, const float *B, const float *vol, int32_t K,
+                            int32_t ldk, int32_t D, float *sino, void *stream);
+mm_status mm_loss_gradient_sparse(const mm_geometry *g, const mm_sparse_plan *plan, const float *B, const float *vol, int32_t K,
+                                  int32_t ldk, int32_t D, const float *data, const float *weights, float *grad, double *loss,
+                                  float *wr_workspace, void *stream);
+
 /* NEXT-3 — regulariser and optimizer building blocks for a device-resident iteration.
  * mm_laplacian: vol_out[x][i] = sum of the six face neighbours of vol[x][i] - 6 vol[x][i], neighbours outside the
  *   volume counting as 0 (reading S21); vol, vol_out [X][Y][Z][ldk] DEVICE, distinct; pad channels written 0.

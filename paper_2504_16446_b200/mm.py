@@ -19,7 +19,7 @@ _lib = None
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
            "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
-           "mm_axpy_precond", "mm_iterate", "mm_workspace_release", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
+           "mm_axpy_precond", "mm_basis_sparsify", "mm_sparse_plan_create", "mm_sparse_plan_destroy", "mm_sparse_plan_info", "mm_forward_sparse", "mm_loss_gradient_sparse", "mm_iterate", "mm_workspace_release", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
 
@@ -79,6 +79,12 @@ def load():
     L.mm_loss_gradient_host.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
     L.mm_host_workspace_release.argtypes = []
     L.mm_workspace_release.argtypes = []
+    L.mm_basis_sparsify.argtypes = [vp, i32, i32, i32, i32, vp]
+    L.mm_sparse_plan_create.argtypes = [vp, vp, i32, i32, ctypes.POINTER(vp)]
+    L.mm_sparse_plan_destroy.argtypes = [vp]
+    L.mm_sparse_plan_info.argtypes = [vp, ctypes.POINTER(i32), dp, vp]
+    L.mm_forward_sparse.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mm_loss_gradient_sparse.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     L.mm_iterate.argtypes = [vp, vp, i32, i32, i32, vp, vp, ctypes.POINTER(_IterParams), vp, vp, vp, ctypes.POINTER(i32), vp]
     L.mm_set_phase_event.argtypes = [vp]
     L.mm_launch_count.restype = i64
@@ -341,6 +347,54 @@ def mm_nesterov_step(c, v, grad, eta: float, momentum: float, stream=None):
     _check(load().mm_nesterov_step(_dev(c, c.shape, "c"), _dev(v, c.shape, "v"), _dev(grad, c.shape, "grad"), float(eta),
                                    float(momentum), c.numel(), _stream(stream)), "mm_nesterov_step")
     return c, v
+
+
+def mm_basis_sparsify(h_B, n_keep: int) -> np.ndarray:
+    """host helper: keep the n_keep largest |B[s][i][c]| of every (s, c) column, zero the rest (reading S26)."""
+    B = np.ascontiguousarray(h_B, dtype=np.float32)
+    out = np.empty_like(B)
+    P, K, D = B.shape
+    _check(load().mm_basis_sparsify(ctypes.c_void_p(B.ctypes.data), P, K, D, int(n_keep), ctypes.c_void_p(out.ctypes.data)), "mm_basis_sparsify")
+    return out
+
+
+class SparsePlan:
+    """Owner of an mm_sparse_plan handle: the per-projection lists of channels with a non-zero row of the HOST matrix h_B."""
+
+    def __init__(self, g: Geometry, h_B):
+        B = np.ascontiguousarray(h_B, dtype=np.float32)
+        assert B.shape[0] == g.P
+        self.K, self.D = int(B.shape[1]), int(B.shape[2])
+        h = ctypes.c_void_p()
+        _check(load().mm_sparse_plan_create(g._h, ctypes.c_void_p(B.ctypes.data), self.K, self.D, ctypes.byref(h)), "mm_sparse_plan_create")
+        self._h = h
+        mx, mean = ctypes.c_int32(), ctypes.c_double()
+        self.counts = np.zeros(g.P, dtype=np.int32)
+        _check(load().mm_sparse_plan_info(self._h, ctypes.byref(mx), ctypes.byref(mean), ctypes.c_void_p(self.counts.ctypes.data)), "mm_sparse_plan_info")
+        self.max_active, self.mean_active = mx.value, mean.value
+
+    def __del__(self):
+        if getattr(self, "_h", None) is not None and _lib is not None:
+            _lib.mm_sparse_plan_destroy(self._h)
+            self._h = None
+
+
+def mm_forward_sparse(g: Geometry, plan: SparsePlan, B, vol, K: int, sino, stream=None):
+    ldk, D = vol.shape[-1], B.shape[-1]
+    _check(load().mm_forward_sparse(g._h, plan._h, _dev(B, (g.P, K, D), "B"), _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, D,
+                                    _dev(sino, g.proj_shape(D), "sino"), _stream(stream)), "mm_forward_sparse")
+    return sino
+
+
+def mm_loss_gradient_sparse(g: Geometry, plan: SparsePlan, B, vol, K: int, data, weights, grad, loss, wr_workspace, stream=None):
+    import torch
+    ldk, D = vol.shape[-1], B.shape[-1]
+    w = ctypes.c_void_p(None) if weights is None else _dev(weights, g.proj_shape(D), "weights")
+    _check(load().mm_loss_gradient_sparse(g._h, plan._h, _dev(B, (g.P, K, D), "B"), _dev(vol, g.vol_shape(ldk), "vol"), K, ldk, D,
+                                          _dev(data, g.proj_shape(D), "data"), w, _dev(grad, g.vol_shape(ldk), "grad"),
+                                          _dev(loss, (1,), "loss", torch.float64),
+                                          _dev(wr_workspace, g.proj_shape(D), "wr_workspace"), _stream(stream)), "mm_loss_gradient_sparse")
+    return grad, loss
 
 
 def mm_iterate(g: Geometry, B, K: int, data, weights, c, v, losses, eta: float, momentum: float = 0.0, mu_laplacian: float = 0.0,

@@ -718,3 +718,45 @@ def test_device_resident_iteration_with_stop_rule(ora, mm, momentum, mu_lap, mu_
     _, _, L6 = ora.iterate(go, B, data, c.w, np.zeros(c.shape + (K,), np.float32), eta, momentum, mu_lap, mu_l2, 6, 0.0)
     torch.cuda.synchronize()
     assert np.abs(l6.cpu().numpy() - np.array(L6)).max() <= TOL_LOSS * max(L6)
+
+
+@pytest.mark.parametrize("kind,K,n_keep", [("nn", 162, None), ("nn", 50, None), ("gk", 50, 2), ("gk", 18, 1), ("sh", 45, 3)])
+def test_sparse_forward_and_gradient(ora, mm, kind, K, n_keep):
+    """NEXT-2 (reading S26): the forward model and the fused gradient with a sparse reciprocal-space map —
+    an NN basis as it is (K = 162, 50: Table V's sizes) or a GK / SH basis thresholded to n_keep coefficients per
+    segment — against the oracle with the same sparse matrix, and against the library's dense calls."""
+    import torch
+    r = np.random.default_rng(K + (n_keep or 0))
+    P, D = 9, 8
+    ldk = synth.ldk_for(K)
+    c = Case((17, 15, 19), (21, 20), r.uniform(0, 2 * math.pi, P), r.uniform(-0.7, 0.7, P), K, ldk, D, seed=K,
+             joff=r.uniform(-1, 1, P), koff=r.uniform(-1, 1, P))
+    go, gm = c.geoms(ora, mm)
+    if kind == "sh":
+        B = mm.mm_basis_sh_matrix(gm, 8, *synth.segments(D))
+    else:
+        B = mm.mm_basis_grid_matrix(gm, mm.MM_BASIS_GK if kind == "gk" else mm.MM_BASIS_NN, synth.grid_directions(K),
+                                    *synth.segments(D), sigma=0.3, n_quad=8)
+    if n_keep is not None:
+        B = mm.mm_basis_sparsify(B, n_keep)
+        assert np.array_equal(B, ora.sparsify_basis(B, n_keep)) and ((B != 0).sum(axis=1) <= n_keep).all()
+    plan = mm.SparsePlan(gm, B)
+    assert plan.max_active < K and plan.max_active <= D * (n_keep or 8)
+    dB, dvol = dev(B), dev(c.vol)
+    model = torch.full(gm.proj_shape(D), float("nan"), device="cuda")
+    mm.mm_forward_sparse(gm, plan, dB, dvol, K, model)
+    want_model = ora.forward(go, B, c.vol[..., :K])
+    scale = float(np.abs(want_model).max())
+    assert einf(model.cpu().numpy(), want_model) <= TOL
+    dense = torch.empty_like(model)
+    mm.mm_forward(gm, dB, dvol, K, dense)
+    assert einf(dense.cpu().numpy(), model.cpu().numpy()) <= 2e-6
+    data = (want_model + 0.05 * scale * c.data).astype(np.float32)
+    grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    loss = torch.full((1,), float("nan"), device="cuda", dtype=torch.float64)
+    wr = torch.full(gm.proj_shape(D), float("nan"), device="cuda")
+    mm.mm_loss_gradient_sparse(gm, plan, dB, dvol, K, dev(data), dev(c.w), grad, loss, wr)
+    L, g_o, wr_o = ora.loss_gradient(go, B, c.vol[..., :K], data, c.w, form="scatter")
+    got = grad.cpu().numpy()
+    assert np.abs(wr.cpu().numpy() - wr_o).max() / scale <= TOL and abs(loss.item() - L) <= TOL_LOSS * L
+    assert einf(got[..., :K], g_o) <= TOL and np.all(got[..., K:] == 0.0)

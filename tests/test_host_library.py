@@ -191,3 +191,22 @@ def test_host_workspace_release_with_nothing_allocated(mm):
     """mm_host_workspace_release is a no-op (MM_OK) before any host call and needs no device."""
     mm.mm_host_workspace_release()
     mm.mm_host_workspace_release()
+
+
+def test_sparsify_and_plan_match_the_oracle(ora, mm):
+    """NEXT-2 host parts (PAPER.md:274, reading S26): mm_basis_sparsify == oracle.sparsify_basis bit for bit, incl. ties;
+    the plan's channel lists are the rows of B with a non-zero entry."""
+    from paper_2504_16446_b200 import synth
+    r = np.random.default_rng(8)
+    B = r.standard_normal((4, 11, 5)).astype(np.float32)
+    B[1, 3] = B[1, 7]                                                  # equal magnitudes: lowest index first
+    for n in (1, 2, 6, 11, 40):
+        assert np.array_equal(mm.mm_basis_sparsify(B, n), ora.sparsify_basis(B, n))
+    g = mm.Geometry((4, 4, 4), (4, 4), [0.3, 1.1, 2.0], [0.2, -0.5, 0.0])
+    Bnn = mm.mm_basis_grid_matrix(g, mm.MM_BASIS_NN, synth.grid_directions(60), *_segs(8), n_quad=4)
+    plan = mm.SparsePlan(g, Bnn)
+    want = (np.abs(Bnn).sum(axis=2) > 0).sum(axis=1)
+    assert np.array_equal(plan.counts, want) and plan.max_active == want.max() and abs(plan.mean_active - want.mean()) < 1e-12
+    assert plan.max_active <= 8 * 4 < 60                               # at most one direction per quadrature point
+    one = mm.SparsePlan(g, mm.mm_basis_sparsify(Bnn, 1))
+    assert one.max_active <= 8
