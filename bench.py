@@ -71,6 +71,8 @@ def record_traffic(csv_path, cfg_name, command):
         if len(r) <= max(ir, iw):
             continue
         b = float(r[ir]) * unit[rows[1][ir]] + float(r[iw]) * unit[rows[1][iw]]
+        if b != b:                                   # a launch ncu could not replay: no figure
+            continue
         for key in ("john_forward_kernel", "adjoint_brick_kernel"):
             if key in r[ik]:
                 ent[key + "_dram_bytes"] = int(b)
@@ -83,7 +85,7 @@ def record_traffic(csv_path, cfg_name, command):
         tr = {}
     tr["source_sha16"] = source_sha16()
     tr["command"] = command
-    tr[cfg_name] = ent
+    tr.setdefault(cfg_name, {}).update(ent)
     with open(out, "w") as f:
         json.dump(tr, f, indent=1)
     print(json.dumps(tr))
