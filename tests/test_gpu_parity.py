@@ -760,3 +760,27 @@ def test_sparse_forward_and_gradient(ora, mm, kind, K, n_keep):
     got = grad.cpu().numpy()
     assert np.abs(wr.cpu().numpy() - wr_o).max() / scale <= TOL and abs(loss.item() - L) <= TOL_LOSS * L
     assert einf(got[..., :K], g_o) <= TOL and np.all(got[..., K:] == 0.0)
+
+
+def test_boundary_errors_and_workspace_release(ora, mm):
+    """robustness at the boundary: unsupported channel strides are refused (not half-written), the scratch pool can be
+    released and refills, and the result after a release is bit-identical."""
+    import torch
+    gm = mm.Geometry((8, 8, 8), (8, 8), [0.2, 1.0], [0.0, 0.3])
+    big = torch.zeros(gm.vol_shape(260), device="cuda")
+    with pytest.raises(mm.MMError, match="not supported"):
+        mm.mm_john_forward(gm, big, 200, torch.zeros(gm.proj_shape(260), device="cuda"))
+    cfg, c = cfg_case("C3", (12, 10, 14), (15, 17), 2, seed=71)
+    go, gm = c.geoms(ora, mm)
+    B = dev(mm.mm_basis_sh_matrix(gm, cfg.ell_max, *synth.segments(c.D)))
+    data = dev(synth.surrogate_model(cfg))
+    out = []
+    for rep in range(2):
+        grad = torch.full(gm.vol_shape(c.ldk), float("nan"), device="cuda")
+        loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+        wr = torch.empty(gm.proj_shape(c.D), device="cuda")
+        mm.mm_loss_gradient(gm, B, dev(c.vol), c.K, data, dev(c.w), grad, loss, wr)     # ldk = 48: pooled copy + pooled operand tiles
+        torch.cuda.synchronize()
+        out.append((grad.clone(), wr.clone()))
+        mm.mm_workspace_release()
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1]) and not torch.isnan(out[0][0]).any().item()
