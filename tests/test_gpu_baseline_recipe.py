@@ -129,3 +129,29 @@ def test_recipe_c5_full_size_sampled(ora, mm):
     """config 5 at FULL size with its own data: Poisson noise at 1e4 counts (1 % residual) on the oracle's sinogram."""
     cfg = synth.get_config("C5")
     _sampled(ora, mm, "C5", 200, _voxel_sample(cfg, 55, 24, 12), seed=5)
+
+
+@pytest.mark.skipif(__import__("os").environ.get("MM_WHOLE_C5") != "1",
+                    reason="11 minutes of oracle time on the host cores and 40 GB of host memory: set MM_WHOLE_C5=1")
+def test_recipe_c5_whole_arrays(ora, mm):
+    """config 5, EVERY gradient entry (not a sample): the oracle's full adjoint of its own weighted residual, in three
+    passes of 15 channels (the K-channel back-projection input is 8.5 GB in fp64 per pass).  Opt-in because of its
+    cost; the figure it printed in round 2 is in DESIGN.md section 6."""
+    cfg, gm, go, B, vol, w, model, data = recipe(ora, mm, "C5")
+    K = cfg.K
+    grad, L, wr = run_gpu(mm, gm, B, vol, K, data, w)
+    wr_o = model - data.astype(np.float64)
+    del model
+    e_wr = float(np.abs(wr.cpu().numpy() - wr_o).max() / np.abs(wr_o).max())
+    got = grad.cpu().numpy()[..., :K].astype(np.float64)
+    del grad, wr
+    Bd = B.astype(np.float64)
+    g_o = np.empty(tuple(cfg.shape) + (K,), dtype=np.float64)
+    for lo in range(0, K, 15):
+        hi = min(K, lo + 15)
+        g_o[..., lo:hi] = ora.john_adjoint(go, np.einsum("sjkc,sic->sjki", wr_o, Bd[:, lo:hi, :]), form="gather")
+    err = np.abs(got - g_o)
+    scale = np.abs(g_o).max()
+    print(f"C5 whole arrays: E_inf(wr) = {e_wr:.3e}, E_inf(grad) = {err.max() / scale:.3e}, rms error / max = "
+          f"{np.sqrt((err ** 2).mean()) / scale:.3e}")
+    assert e_wr <= TOL and err.max() / scale <= TOL
