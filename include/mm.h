@@ -291,6 +291,24 @@ mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const fl
                                 int32_t ldk, int32_t D, const float *h_data, const float *h_weights,
                                 float *h_grad, double *h_loss);
 
+/* A^T (a6 + a7) for callers that may not allocate: code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc.  Same arguments, kernels (bop_prep_kernel + adjoint_brick_kernel) and result as
+ * mm_adjoint on the shapes the brick kernel serves, but the one piece of scratch it needs — the split operand tiles
+ * of w_s B_s, P * 2 * npad(ldk) * D * 4 bytes with npad = ldk rounded up to 16/32/48/64/96/128/192 — lives in a
+ * static device array of MM_ADJOINT_NOALLOC_MAX_BYTES inside the library (held on every GPU that loads it until the
+ * process exits) instead of the stream-ordered pool.  The call makes no cudaMalloc/cudaFree/pool call of any kind.
+ *   - MM_ERR_UNSUPPORTED (nothing enqueued) if the scratch would exceed the maximum, or the shape is not the brick
+ *     kernel's: D = 8 or 16, ldk % 4 == 0, ldk <= 192, 16-byte aligned B / sino / vol_out, a geometry whose brick
+ *     shadow fits a 16 x 17 pixel tile (every standard tomographic geometry).  There is no fallback: use mm_adjoint.
+ *     Config 5 needs 1.1 MB (P = 360, ldk = 48, D = 8), config 4 2.0 MB (P = 500, ldk = 32, D = 16).
+ *   - All calls share the array.  Every element the kernel reads is rewritten by the call itself, so a call never
+ *     sees an earlier call's contents; but two calls whose kernels can overlap on the GPU (different streams, no
+ *     dependency) race on it: serialise them (one stream, or an event between them).
+ *   - vol_out [X][Y][Z][ldk] is overwritten; asynchronous on `stream` like every device call here. */
+#define MM_ADJOINT_NOALLOC_MAX_BYTES (4u << 20)
+mm_status mm_adjoint_noalloc(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk,
+                             int32_t D, float *vol_out, void *stream);
+
 /* Number of kernel launches this library has enqueued since load (for bench accounting). */
 int64_t mm_launch_count(void);
 

@@ -26,6 +26,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+#include <mutex>
+#include <string>
+
 #include "mm_internal.h"
 #include "mm_ptx.cuh"
 
@@ -448,4 +452,114 @@ int mm_adjoint_brick_launch(const mm_geometry *g, const AdjArgs &a, void *stream
 #undef MM_BRICK_CASE
     const cudaError_t e2 = mm_scratch_free(bop, st);
     return e != cudaSuccess ? e : e2;
+}
+
+// ================================================================================================
+// mm_adjoint_noalloc: the same brick adjoint for callers that may not allocate (include/mm.h)
+// ================================================================================================
+// The one piece of scratch the brick adjoint needs is the split operand tiles of w_s B_s (bop_prep_kernel's output,
+// P x 2 x NPAD x D floats: 1.1 MB on config 5).  Here they live in a file-scope device array instead of the pool:
+// every GPU that loads the library holds MM_ADJOINT_NOALLOC_MAX_BYTES until the process exits.  All calls share the
+// array; bop_prep_kernel rewrites every element the brick kernel reads (rows K..NPAD-1 as zeros), so nothing carried
+// over from an earlier call is ever used — but two calls in flight on the GPU at once (different streams) race on it.
+static __device__ __align__(256) float g_bop_static[MM_ADJOINT_NOALLOC_MAX_BYTES / sizeof(float)];
+
+namespace {
+// `g_bop_static` in host code names a host-side shadow, not device memory: the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int MAX_DEVICES = 64;
+float *g_bop_static_addr[MAX_DEVICES];          // guarded by the acquire/release pair below
+std::atomic<int> g_bop_static_ready[MAX_DEVICES];
+
+cudaError_t static_bop_address(int dev, float **out)
+{
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+    if (!g_bop_static_ready[dev].load(std::memory_order_acquire)) {
+        static std::mutex mu;
+        std::lock_guard<std::mutex> lock(mu);
+        if (!g_bop_static_ready[dev].load(std::memory_order_relaxed)) {
+            int cur = -1;
+            cudaError_t e = cudaGetDevice(&cur);
+            if (e != cudaSuccess) return e;
+            if (cur != dev) return cudaErrorInvalidDevice;          // the caller checked; never look a symbol up on another device
+            float *p = nullptr;
+            e = cudaGetSymbolAddress((void **)&p, g_bop_static);
+            if (e != cudaSuccess) return e;
+            if (!p || (reinterpret_cast<uintptr_t>(p) & 255u) != 0) return cudaErrorInvalidSymbol;
+            g_bop_static_addr[dev] = p;
+            g_bop_static_ready[dev].store(1, std::memory_order_release);
+        }
+    }
+    *out = g_bop_static_addr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" mm_status mm_adjoint_noalloc(const mm_geometry *g, const float *B, const float *sino, int32_t K, int32_t ldk,
+                                        int32_t D, float *vol_out, void *stream)
+{
+    const char *who = "mm_adjoint_noalloc";
+    if (!g) { mm_set_error(std::string(who) + ": NULL geometry"); return MM_ERR_NULL; }
+    if (!g->d_table) { mm_set_error(std::string(who) + ": geometry was created without a CUDA device (no CPU fallback)"); return MM_ERR_CUDA; }
+    if (!B || !sino || !vol_out) { mm_set_error(std::string(who) + ": NULL buffer"); return MM_ERR_NULL; }
+    if (K < 1 || ldk < K || D < 1 || D > MM_MAX_D) { mm_set_error(std::string(who) + ": need 1 <= K <= ldk, 1 <= D <= MM_MAX_D"); return MM_ERR_SHAPE; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != g->device) {
+        cudaGetLastError();
+        mm_set_error(std::string(who) + ": the geometry was created on CUDA device " + std::to_string(g->device) +
+                     ", the current device is " + std::to_string(dev));
+        return MM_ERR_VALUE;
+    }
+    AdjArgs a;
+    a.tab = g->d_table; a.src = sino; a.B = B; a.out = vol_out; a.K = K; a.ldk = ldk; a.D = D;
+    a.X = g->shape[0]; a.Y = g->shape[1]; a.Z = g->shape[2]; a.J = g->J; a.Kd = g->Kd; a.P = g->P;
+    a.bilinear = 0; a.vox_begin = 0; a.vox_end = (long long)a.X * a.Y * a.Z;
+    a.vec_ok = (D % 4 == 0) && (reinterpret_cast<uintptr_t>(sino) & 15u) == 0;
+    const int NP = npad_for(ldk);
+    const size_t need = (size_t)a.P * 2 * NP * D * sizeof(float);
+    if (need > (size_t)MM_ADJOINT_NOALLOC_MAX_BYTES) {
+        mm_set_error(std::string(who) + ": P * 2 * npad(ldk) * D * 4 = " + std::to_string(need) + " bytes of operand scratch exceed the static " +
+                     std::to_string((size_t)MM_ADJOINT_NOALLOC_MAX_BYTES) + " bytes (MM_ADJOINT_NOALLOC_MAX_BYTES); use mm_adjoint");
+        return MM_ERR_UNSUPPORTED;
+    }
+    if (!mm_adjoint_brick_supported(g, a)) {
+        mm_set_error(std::string(who) + ": only the brick kernel's shapes are served without allocation (D = 8 or 16, ldk % 4 == 0, "
+                     "ldk <= 192, 16-byte aligned buffers, a geometry whose brick shadow fits a 16 x 17 pixel tile); use mm_adjoint");
+        return MM_ERR_UNSUPPORTED;
+    }
+    float *bop = nullptr;
+    cudaError_t e = static_bop_address(dev, &bop);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        mm_set_error(std::string(who) + ": cudaGetSymbolAddress(static scratch): " + cudaGetErrorString(e));
+        return MM_ERR_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    BrickArgs b;
+    b.tab = a.tab; b.out = a.out; b.ldk = a.ldk; b.X = a.X; b.Y = a.Y; b.Z = a.Z; b.P = a.P;
+    b.x_begin = 0; b.x_end = a.X;
+    b.nby = (a.Y + BY - 1) / BY; b.nbz = (a.Z + BZ - 1) / BZ;
+    b.tj = g->brick_tj; b.tk = g->brick_tk;
+    b.tile_stride = (b.tj * b.tk * a.D * 4 + 1023) & ~1023;
+    b.bilinear = 0;
+    b.bop = bop;
+    alignas(64) CUtensorMap tmap;
+    const unsigned long long n[4] = {(unsigned long long)a.D, (unsigned long long)a.Kd, (unsigned long long)a.J, (unsigned long long)a.P};
+    const unsigned box[4] = {(unsigned)a.D, (unsigned)b.tk, (unsigned)b.tj, 1u};
+    if (!mm_tma_encode_4d_f32(&tmap, a.src, n, box, a.D * 4)) { mm_set_error(std::string(who) + ": tensor map encode failed"); return MM_ERR_CUDA; }
+    bop_prep_kernel<<<a.P, 128, 0, st>>>(a.B, a.tab, bop, a.K, a.D, NP);      // rewrites every element the brick kernel reads
+    e = cudaGetLastError();
+#define MM_BRICK_CASE(DD, NN) if (e == cudaSuccess && a.D == DD && NP == NN) e = launch_brick<DD, NN>(tmap, b, st)
+    MM_BRICK_CASE(8, 16); MM_BRICK_CASE(8, 32); MM_BRICK_CASE(8, 48); MM_BRICK_CASE(8, 64);
+    MM_BRICK_CASE(8, 96); MM_BRICK_CASE(8, 128); MM_BRICK_CASE(8, 192);
+    MM_BRICK_CASE(16, 16); MM_BRICK_CASE(16, 32); MM_BRICK_CASE(16, 48); MM_BRICK_CASE(16, 64);
+    MM_BRICK_CASE(16, 96); MM_BRICK_CASE(16, 128); MM_BRICK_CASE(16, 192);
+#undef MM_BRICK_CASE
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        mm_set_error(std::string(who) + ": " + cudaGetErrorString(e));
+        return MM_ERR_CUDA;
+    }
+    mm_note_launches(2);                                                       // bop_prep_kernel + adjoint_brick_kernel
+    return MM_OK;
 }

@@ -18,7 +18,7 @@ _lib = None
 
 SYMBOLS = ["mm_geometry_create", "mm_geometry_destroy", "mm_geometry_get", "mm_basis_sh_matrix", "mm_basis_sh_matrix_2theta", "mm_basis_grid_matrix",
            "mm_john_forward", "mm_john_adjoint", "mm_basis_forward", "mm_basis_adjoint", "mm_forward",
-           "mm_adjoint", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
+           "mm_adjoint", "mm_adjoint_noalloc", "mm_john_backproject", "mm_backproject", "mm_loss_gradient", "mm_loss_gradient_huber", "mm_residual_loss", "mm_reciprocal",
            "mm_axpy_precond", "mm_basis_sparsify", "mm_sparse_plan_create", "mm_sparse_plan_destroy", "mm_sparse_plan_info", "mm_forward_sparse", "mm_loss_gradient_sparse", "mm_iterate", "mm_workspace_release", "mm_laplacian", "mm_regulariser", "mm_nesterov_step", "mm_derived_quantities", "mm_axpy", "mm_loss_gradient_host", "mm_host_workspace_release", "mm_launch_count", "mm_set_phase_event",
            "mm_status_string", "mm_last_error"]
 
@@ -64,6 +64,7 @@ def load():
     L.mm_basis_adjoint.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_forward.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_adjoint.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mm_adjoint_noalloc.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_john_backproject.argtypes = [vp, vp, i32, i32, vp, vp]
     L.mm_backproject.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     L.mm_loss_gradient.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
@@ -249,6 +250,17 @@ def mm_adjoint(g: Geometry, B, sino, K: int, vol_out, stream=None):
     ldk, D = vol_out.shape[-1], B.shape[-1]
     _check(load().mm_adjoint(g._h, _dev(B, (g.P, K, D), "B"), _dev(sino, g.proj_shape(D), "sino"), K, ldk, D,
                              _dev(vol_out, g.vol_shape(ldk), "vol_out"), _stream(stream)), "mm_adjoint")
+    return vol_out
+
+
+ADJOINT_NOALLOC_MAX_BYTES = 4 << 20            # MM_ADJOINT_NOALLOC_MAX_BYTES of include/mm.h
+
+
+def mm_adjoint_noalloc(g: Geometry, B, sino, K: int, vol_out, stream=None):
+    """mm_adjoint without any allocation: operand scratch in the library's static device array (include/mm.h)."""
+    ldk, D = vol_out.shape[-1], B.shape[-1]
+    _check(load().mm_adjoint_noalloc(g._h, _dev(B, (g.P, K, D), "B"), _dev(sino, g.proj_shape(D), "sino"), K, ldk, D,
+                                     _dev(vol_out, g.vol_shape(ldk), "vol_out"), _stream(stream)), "mm_adjoint_noalloc")
     return vol_out
 
 
