@@ -50,6 +50,9 @@ extern "C" mm_status mm_set_phase_event(void *cuda_event)
 #ifndef FWD_MIX48
 #define FWD_MIX48 1
 #endif
+#ifndef FWD_COMMON_START
+#define FWD_COMMON_START 1              // cooperative march: the rays of a block start at the block's first slab
+#endif
 #ifndef FWD_TK
 #define FWD_TK 4                        // rays along k in the tile of a 32-ray block
 #endif
@@ -288,16 +291,28 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
         const int ldk4 = a.ldk / VEC;
         const int sM4 = (int)(sM / VEC), sU4 = (int)(sU / VEC), sV4 = (int)(sV / VEC);
         const int zero_off = LERP ? a.zero_vox * ldk4 : 0;
-        int rounds = (n1 >= n0) ? (n1 - n0 + G) / G : 0;
+        // All rays of the block start at the block's first slab (slabs before a ray's own n0 carry zero weights):
+        // neighbouring rays are then at the SAME slab in the same round and find each other's taps in L1.  With
+        // every ray starting at its own n0 they were up to a tile's width of slabs apart (FWD_COMMON_START).
+        int nstart = n0;
+        if constexpr (FWD_COMMON_START && LERP) {                 // measured on the ldk = 48 path only (config 5: -4 %)
+            __shared__ int s_nbeg;
+            if (tid == 0) s_nbeg = 0x7fffffff;
+            __syncthreads();
+            if (q == 0 && n1 >= n0) atomicMin(&s_nbeg, n0);
+            __syncthreads();
+            nstart = s_nbeg;
+        }
+        int rounds = (n1 >= n0) ? (n1 - nstart + G) / G : 0;
         rounds = __reduce_max_sync(0xffffffffu, rounds);          // the warp's groups step through rounds together
         for (int rd = 0; rd < rounds; rd++) {
-            const int nb = n0 + rd * G;
+            const int nb = nstart + rd * G;
             {   // lane q: taps of slab nb + q
                 const int n = nb + q;
                 SlabTaps t;
                 t.o00 = t.o10 = t.o01 = t.o11 = 0;
                 t.w00 = t.w10 = t.w01 = t.w11 = 0.f;
-                if (n <= n1) {
+                if (n >= n0 && n <= n1) {
                     // 24.40 fixed point: the integer part is the tap index, the fraction the bilinear weight
                     const long long pu = pu0 + (long long)n * su_fx, pv = pv0 + (long long)n * sv_fx;
                     const int iu = (int)(pu >> FX_BITS), iv = (int)(pv >> FX_BITS);
