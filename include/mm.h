@@ -212,7 +212,11 @@ mm_status mm_derived_quantities(const mm_geometry *g, const float *vol, int32_t 
  *   mm_forward_sparse       = mm_forward with that B, marching only the active channels of each projection.
  *   mm_loss_gradient_sparse = mm_loss_gradient with that B: sparse phase 1, dense tensor-core contraction in phase 2.
  * B (DEVICE) must have the zero pattern the plan was made from: rows outside the lists are never read.  Results equal
- * the dense calls' on the same B to fp32 rounding. */
+ * the dense calls' on the same B to fp32 rounding.
+ * With at most 32 active channels per projection the march runs on channel-planar, zero-padded copies of `vol` that the
+ * call makes itself in the library's scratch pool (K planes of (X+4)(Y+4)(Z+4) floats, one set per family of major
+ * axes in use: up to 2.2 x the volume), so that only the active channels' planes are read; otherwise, or if the pool
+ * cannot supply the copies, it runs on `vol` as it is (same results to rounding, no scratch). */
 typedef struct mm_sparse_plan mm_sparse_plan;
 mm_status mm_basis_sparsify(const float *h_B, int32_t P, int32_t K, int32_t D, int32_t n_keep, float *h_B_out);
 mm_status mm_sparse_plan_create(const mm_geometry *g, const float *h_B, int32_t K, int32_t D, mm_sparse_plan **out);
@@ -285,7 +289,8 @@ mm_status mm_axpy(float *c, const float *grad, float eta, int64_t n, void *strea
 mm_status mm_host_workspace_release(void);
 /* Also returns to the driver the device memory cached in the library's stream-ordered scratch pool (see "stream"
  * above): the adjoint's split operand tiles (P*ldk*D*8 bytes), the forward's repacked volume when ldk = 48 (one
- * volume), mm_iterate's work arrays.  The pool refills on the next call that needs it. */
+ * volume), the sparse forward's channel-planar copies, mm_iterate's work arrays.  The pool refills on the next call
+ * that needs it. */
 mm_status mm_workspace_release(void);
 mm_status mm_loss_gradient_host(const mm_geometry *g, const float *h_B, const float *h_vol, int32_t K,
                                 int32_t ldk, int32_t D, const float *h_data, const float *h_weights,

@@ -88,6 +88,11 @@ bool mm_tma_encode_4d_f32(void *tmap_out, const void *base, const unsigned long 
 // mm_adjoint_brick.cu: fused adjoint, voxel bricks + TMA-staged detector tiles + tcgen05 (3xTF32), the primary path
 bool mm_adjoint_brick_supported(const mm_geometry *g, const AdjArgs &a);
 int mm_adjoint_brick_launch(const mm_geometry *g, const AdjArgs &a, void *stream);   // returns a cudaError_t
+// mm_sparse_planar.cu: the sparse forward on channel-planar copies of the volume (returns a cudaError_t)
+bool mm_sparse_planar_supported(const mm_geometry *g, int K, int ldk, int max_active);
+int mm_sparse_planar_launch(const mm_geometry *g, const int *d_idx, const int *d_count, int slots, int max_active, const float *B,
+                            const float *vol, int K, int ldk, int D, const float *data, const float *weights, float *sino,
+                            double *loss, int mode, void *stream);
 
 // mm_adjoint_tc.cu: fused adjoint with the basis contraction on the tensor cores (tcgen05, 3xTF32).
 bool mm_adjoint_tc_supported(const AdjArgs &a);

@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include <algorithm>
 #include <new>
@@ -212,8 +213,16 @@ __global__ void __launch_bounds__(256) john_forward_sparse_kernel(const SparseAr
 }
 
 template <int MODE>
-mm_status launch_sparse(const SparseArgs &a, cudaStream_t st)
+mm_status launch_sparse(const SparseArgs &a, cudaStream_t st, const mm_geometry *g = nullptr, const mm_sparse_plan *p = nullptr)
 {
+    // first choice: the march on channel-planar copies (mm_sparse_planar.cu); MM_DISABLE_PLANAR keeps the record layout
+    static const bool planar_off = getenv("MM_DISABLE_PLANAR") != nullptr;
+    if (g && p && !planar_off && mm_sparse_planar_supported(g, a.K, a.ldk, p->max_active)) {
+        const cudaError_t e = (cudaError_t)mm_sparse_planar_launch(g, a.idx, a.count, a.slots, p->max_active, a.B, a.vol, a.K, a.ldk, a.D,
+                                                                   a.data, a.weights, a.sino, a.loss, MODE, st);
+        if (e == cudaSuccess) return MM_OK;
+        cudaGetLastError();                                         // e.g. no scratch for the copies: the kernel below needs none
+    }
     const long long tiles = (long long)a.P * ((a.J + 1) / 2) * ((a.Kd + 3) / 4);
     const int nq = a.slots / 32;
 #define MM_SP_CASE(NQ, DM) john_forward_sparse_kernel<NQ, DM, MODE><<<(unsigned)tiles, 256, 0, st>>>(a)
@@ -349,7 +358,7 @@ extern "C" mm_status mm_forward_sparse(const mm_geometry *g, const mm_sparse_pla
     SparseArgs a;
     fill_sparse(a, g, p, B, vol, K, ldk, D);
     a.sino = sino;
-    return launch_sparse<1>(a, (cudaStream_t)stream);
+    return launch_sparse<1>(a, (cudaStream_t)stream, g, p);
 }
 
 extern "C" mm_status mm_loss_gradient_sparse(const mm_geometry *g, const mm_sparse_plan *p, const float *B, const float *vol, int32_t K,
@@ -367,7 +376,7 @@ extern "C" mm_status mm_loss_gradient_sparse(const mm_geometry *g, const mm_spar
     SparseArgs a;
     fill_sparse(a, g, p, B, vol, K, ldk, D);
     a.data = data; a.weights = weights; a.sino = wr_workspace; a.loss = loss;
-    st = launch_sparse<2>(a, cs);                                   // phase 1: active channels only
+    st = launch_sparse<2>(a, cs, g, p);                             // phase 1: active channels only
     if (st != MM_OK) return st;
     return mm_adjoint(g, B, wr_workspace, K, ldk, D, grad, stream);  // phase 2: dense contraction on the tensor cores
 }

@@ -744,7 +744,11 @@ def test_sparse_forward_and_gradient(ora, mm, kind, K, n_keep):
     assert plan.max_active < K and plan.max_active <= D * (n_keep or 8)
     dB, dvol = dev(B), dev(c.vol)
     model = torch.full(gm.proj_shape(D), float("nan"), device="cuda")
+    launches = mm.mm_launch_count()
     mm.mm_forward_sparse(gm, plan, dB, dvol, K, model)
+    launches = mm.mm_launch_count() - launches
+    # <= 32 active channels: the march on channel-planar copies (transposes + march); more: the record-layout kernel
+    assert launches >= 2 if plan.max_active <= 32 else launches == 1
     want_model = ora.forward(go, B, c.vol[..., :K])
     scale = float(np.abs(want_model).max())
     assert einf(model.cpu().numpy(), want_model) <= TOL
