@@ -46,13 +46,12 @@ def algorithmic_bytes(cfg):
 
 
 def source_sha16():
-    """hash of the kernel sources: ties a stored ncu traffic figure to the code it was measured on"""
-    import glob
+    """hash of the sources of the step's two kernels (john_forward_kernel, adjoint_brick_kernel) and of the headers they
+    include: ties a stored ncu traffic figure to the code it was measured on"""
     import hashlib
     h = hashlib.sha256()
-    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", "*.cu*")) +
-                    glob.glob(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", "*.h"))):
-        with open(f, "rb") as fh:
+    for name in ("mm_adjoint_brick.cu", "mm_internal.h", "mm_kernels.cu", "mm_ptx.cuh"):
+        with open(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", name), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
 
