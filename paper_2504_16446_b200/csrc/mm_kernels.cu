@@ -136,29 +136,6 @@ __device__ __forceinline__ void ldg_nc_vec(const float *p, float (&v)[VEC])
     }
 }
 
-// Packed fp32 pairs (sm_100: add/sub/fma .f32x2 -> FADD2/FFMA2): two adjacent channels in one 64-bit register.
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-// read-only 32- and 16-byte loads as pairs, in program order like ldg_nc_vec
-__device__ __forceinline__ void ldg_nc_pairs4(const float *p, f32x2 (&v)[4])
-{
-    asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v[0]), "=l"(v[1]), "=l"(v[2]), "=l"(v[3]) : "l"(p));
-}
-__device__ __forceinline__ void ldg_nc_pairs2(const float *p, f32x2 (&v)[2])
-{
-    asm volatile("ld.global.nc.v2.b64 {%0,%1}, [%2];" : "=l"(v[0]), "=l"(v[1]) : "l"(p));
-}
-// bilinear value of a pair of channels from its four taps as nested differences: c00 + fu (c10 - c00), ... (see LERP)
-__device__ __forceinline__ f32x2 lerp2(f32x2 c00, f32x2 c10, f32x2 c01, f32x2 c11, f32x2 fu, f32x2 fv)
-{
-    const f32x2 t0 = fma2(fu, sub2(c10, c00), c00), t1 = fma2(fu, sub2(c11, c01), c01);
-    return fma2(fv, sub2(t1, t0), t0);
-}
-
 // keep the slabs n in [lo,hi] on which -1 < A + n*s < N can hold (one slab of slack on each side)
 __device__ __forceinline__ void clip_range(double A, double s, int N, double &lo, double &hi)
 {
@@ -204,7 +181,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     // tap on average against 3 for three 64-byte pieces (a load costs one L1 wavefront per distinct line).
     constexpr bool MIX = FWD_MIX48 && VEC == 4 && G == 4 && NQ == 3;
     // LERP (MIX only; the volume is the library's own copy with an all-zero record appended): the bilinear value of a
-    // slab is formed as nested differences, c00 + fu (c10 - c00) etc., in packed fp32 pairs.  A constant (or slowly
+    // slab is formed as nested differences, c00 + fu (c10 - c00) etc. (scalar fp32; see the march below).  A constant (or slowly
     // varying) field is then reproduced exactly, so a run of slabs through a uniform region adds exact multiples of
     // the voxel value.  Four weighted FMAs make the partial sums of such a run approach powers of two from below,
     // where round-to-nearest is one-sided: a bias of ~-0.2 ulp per slab, coherent over all rays and amplified by A^T
@@ -249,14 +226,7 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
     for (int t = 0; t < NQ; t++)
 #pragma unroll
         for (int x = 0; x < VEC; x++) { acc[t][x] = 0.f; tot[t][x] = 0.0; }
-    f32x2 acc2[LERP ? 6 : 1];                     // LERP: the same twelve round sums as packed pairs
-#pragma unroll
-    for (int i = 0; i < (LERP ? 6 : 1); i++) acc2[i] = 0ull;
     auto flush = [&]() {
-        if constexpr (LERP) {
-#pragma unroll
-            for (int i = 0; i < 6; i++) { unpack2(acc2[i], acc[i / 2][2 * (i % 2)], acc[i / 2][2 * (i % 2) + 1]); acc2[i] = 0ull; }
-        }
 #pragma unroll
         for (int t = 0; t < NQ; t++)
 #pragma unroll
@@ -356,38 +326,60 @@ __global__ void __launch_bounds__(256, (COOP && (VEC == 8 || NQ >= 3)) ? FWD_MIN
                 }
                 if constexpr (LERP) {
                     const float *base = a.vol + 8 * q, *base2 = a.vol + 32 + 4 * q;
-#pragma unroll
-                    for (int hh = 0; hh < U; hh += 2) {           // 32-byte pieces, two slabs at a time
-                        f32x2 c[2][4][4];
-#pragma unroll
-                        for (int uu = 0; uu < 2; uu++) {
-                            ldg_nc_pairs4(base + (long long)o[hh + uu].x * 4, c[uu][0]);
-                            ldg_nc_pairs4(base + (long long)o[hh + uu].y * 4, c[uu][1]);
-                            ldg_nc_pairs4(base + (long long)o[hh + uu].z * 4, c[uu][2]);
-                            ldg_nc_pairs4(base + (long long)o[hh + uu].w * 4, c[uu][3]);
-                        }
-                        if (hh == 0) flush();                     // the previous step's sums, under this step's load latency
+                    // the round's three load batches (64 registers each): channels 0-31 of slabs 0-1 and of slabs 2-3,
+                    // channels 32-47 of all four slabs.  Scalar arithmetic on purpose: the same sub / fma / add sequence
+                    // in packed pairs (FADD2 / FFMA2, 42 instead of 84 instructions per lane and slab) is bit-identical
+                    // and 5 % SLOWER (config 5: 190.8 against 180.5 ms) — the march waits on latency, not on issue slots,
+                    // and the packed chains are longer.
+                    float cA[2][4][8], cC[U][4][4];
+                    auto load_fh = [&](int hh) {
 #pragma unroll
                         for (int uu = 0; uu < 2; uu++) {
-                            const f32x2 fu = pack2(w[hh + uu].x, w[hh + uu].x), fv = pack2(w[hh + uu].y, w[hh + uu].y);
-#pragma unroll
-                            for (int x = 0; x < 4; x++) acc2[x] = add2(acc2[x], lerp2(c[uu][0][x], c[uu][1][x], c[uu][2][x], c[uu][3][x], fu, fv));
+                            ldg_nc_vec<8>(base + (long long)o[hh + uu].x * 4, cA[uu][0]);
+                            ldg_nc_vec<8>(base + (long long)o[hh + uu].y * 4, cA[uu][1]);
+                            ldg_nc_vec<8>(base + (long long)o[hh + uu].z * 4, cA[uu][2]);
+                            ldg_nc_vec<8>(base + (long long)o[hh + uu].w * 4, cA[uu][3]);
                         }
-                    }
-                    f32x2 c[U][4][2];                             // 16-byte pieces
+                    };
+                    auto math_fh = [&](int hh) {
 #pragma unroll
-                    for (int uu = 0; uu < U; uu++) {
-                        ldg_nc_pairs2(base2 + (long long)o[uu].x * 4, c[uu][0]);
-                        ldg_nc_pairs2(base2 + (long long)o[uu].y * 4, c[uu][1]);
-                        ldg_nc_pairs2(base2 + (long long)o[uu].z * 4, c[uu][2]);
-                        ldg_nc_pairs2(base2 + (long long)o[uu].w * 4, c[uu][3]);
-                    }
+                        for (int uu = 0; uu < 2; uu++) {
+                            const float fu = w[hh + uu].x, fv = w[hh + uu].y;
 #pragma unroll
-                    for (int uu = 0; uu < U; uu++) {
-                        const f32x2 fu = pack2(w[uu].x, w[uu].x), fv = pack2(w[uu].y, w[uu].y);
+                            for (int x = 0; x < 8; x++) {
+                                const float t0 = fmaf(fu, cA[uu][1][x] - cA[uu][0][x], cA[uu][0][x]);
+                                const float t1 = fmaf(fu, cA[uu][3][x] - cA[uu][2][x], cA[uu][2][x]);
+                                acc[x / 4][x % 4] += fmaf(fv, t1 - t0, t0);
+                            }
+                        }
+                    };
+                    auto load_up = [&]() {
 #pragma unroll
-                        for (int x = 0; x < 2; x++) acc2[4 + x] = add2(acc2[4 + x], lerp2(c[uu][0][x], c[uu][1][x], c[uu][2][x], c[uu][3][x], fu, fv));
-                    }
+                        for (int uu = 0; uu < U; uu++) {
+                            ldg_nc_vec<4>(base2 + (long long)o[uu].x * 4, cC[uu][0]);
+                            ldg_nc_vec<4>(base2 + (long long)o[uu].y * 4, cC[uu][1]);
+                            ldg_nc_vec<4>(base2 + (long long)o[uu].z * 4, cC[uu][2]);
+                            ldg_nc_vec<4>(base2 + (long long)o[uu].w * 4, cC[uu][3]);
+                        }
+                    };
+                    auto math_up = [&]() {
+#pragma unroll
+                        for (int uu = 0; uu < U; uu++) {
+                            const float fu = w[uu].x, fv = w[uu].y;
+#pragma unroll
+                            for (int x = 0; x < 4; x++) {
+                                const float t0 = fmaf(fu, cC[uu][1][x] - cC[uu][0][x], cC[uu][0][x]);
+                                const float t1 = fmaf(fu, cC[uu][3][x] - cC[uu][2][x], cC[uu][2][x]);
+                                acc[2][x] += fmaf(fv, t1 - t0, t0);
+                            }
+                        }
+                    };
+                    static_assert(U == 4, "the nested-difference march consumes rounds of four slabs");
+                    load_fh(0);
+                    flush();                                      // the previous round's sums, under this round's load latency
+                    math_fh(0);
+                    load_fh(2); math_fh(2);
+                    load_up(); math_up();
                 } else if constexpr (MIX) {
                     const float *base = a.vol + 8 * q, *base2 = a.vol + 32 + 4 * q;
 #pragma unroll
