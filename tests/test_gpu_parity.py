@@ -766,6 +766,40 @@ def test_sparse_forward_and_gradient(ora, mm, kind, K, n_keep):
     assert einf(got[..., :K], g_o) <= TOL and np.all(got[..., K:] == 0.0)
 
 
+def test_sparse_planar_all_major_axes(ora, mm):
+    """the channel-planar sparse march with all three major axes in one geometry (tilts up to 63 degrees make y the
+    major axis of some projections: copy Z marched along y, besides x on copy Z and z on copy X), a ragged detector
+    (tiles of 32 x 4 rays with tails) and non-cubic volume"""
+    import torch
+    r = np.random.default_rng(77)
+    K, D, P = 50, 8, 14
+    ldk = synth.ldk_for(K)
+    tilts = np.concatenate([r.uniform(-1.1, 1.1, P - 4), [1.05, -1.0, 0.0, 0.79]])
+    c = Case((13, 18, 11), (37, 9), r.uniform(0, 2 * math.pi, P), tilts, K, ldk, D, seed=78,
+             joff=r.uniform(-1, 1, P), koff=r.uniform(-1, 1, P))
+    go, gm = c.geoms(ora, mm)
+    majors = {go.get(s)[3] for s in range(P)}
+    assert majors == {0, 1, 2}
+    B = mm.mm_basis_grid_matrix(gm, mm.MM_BASIS_NN, synth.grid_directions(K), *synth.segments(D), sigma=0.3, n_quad=8)
+    plan = mm.SparsePlan(gm, B)
+    assert plan.max_active <= 32
+    dB, dvol = dev(B), dev(c.vol)
+    model = torch.full(gm.proj_shape(D), float("nan"), device="cuda")
+    launches = mm.mm_launch_count()
+    mm.mm_forward_sparse(gm, plan, dB, dvol, K, model)
+    assert mm.mm_launch_count() - launches == 3                       # two transposes + the march
+    want = ora.forward(go, B, c.vol[..., :K])
+    assert einf(model.cpu().numpy(), want) <= TOL
+    data = (want + 0.05 * float(np.abs(want).max()) * c.data).astype(np.float32)
+    grad = torch.full(gm.vol_shape(ldk), float("nan"), device="cuda")
+    loss = torch.full((1,), float("nan"), device="cuda", dtype=torch.float64)
+    wr = torch.full(gm.proj_shape(D), float("nan"), device="cuda")
+    mm.mm_loss_gradient_sparse(gm, plan, dB, dvol, K, dev(data), dev(c.w), grad, loss, wr)
+    L, g_o, wr_o = ora.loss_gradient(go, B, c.vol[..., :K], data, c.w, form="scatter")
+    assert np.abs(wr.cpu().numpy() - wr_o).max() / float(np.abs(want).max()) <= TOL and abs(loss.item() - L) <= TOL_LOSS * L
+    assert einf(grad.cpu().numpy()[..., :K], g_o) <= TOL
+
+
 def test_boundary_errors_and_workspace_release(ora, mm):
     """robustness at the boundary: unsupported channel strides are refused (not half-written), the scratch pool can be
     released and refills, and the result after a release is bit-identical."""
