@@ -426,6 +426,73 @@ def ours(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def iterate_extra(args):
+    """`--iterate-extra`: NEXT-3 measurement (not the headline step).  The device-resident regularised Nesterov iteration
+    `mm_iterate` on the configured workload (default C5): wall time per iteration for a run of `--steps` iterations with
+    the Laplacian and L2 regularisers and the relative-change stop test every iteration (tol so small that it never
+    fires), against the bare fused gradient timed the same way."""
+    import torch
+    from paper_2504_16446_b200 import mm
+    torch.cuda.set_device(0)
+    mm.load()
+    cfg = synth.get_config(args.config)
+    K, D, ldk = cfg.K, cfg.D, synth.ldk_for(cfg.K)
+    rot, tilt = synth.angles(cfg)
+    g = mm.Geometry(cfg.shape, cfg.det, rot, tilt)
+    B = torch.from_numpy(mm.mm_basis_sh_matrix(g, cfg.ell_max, *synth.segments(D))).cuda()
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed)
+    truth = torch.rand(g.vol_shape(ldk), device="cuda", generator=gen)
+    truth[..., K:] = 0
+    data = torch.empty(g.proj_shape(D), device="cuda")
+    mm.mm_forward(g, B, truth, K, data)
+    scale = float(data.abs().max())
+    del truth
+    n_it = max(2, args.steps)
+    c = torch.zeros(g.vol_shape(ldk), device="cuda")
+    v = torch.zeros_like(c)
+    losses = torch.zeros(n_it, device="cuda", dtype=torch.float64)
+    # step length: a fifth of the exact line-search step along the first gradient, ||g||^2 / ||A g||^2 >= 1 / ||A^T A||
+    g0 = torch.empty_like(c)
+    l0 = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr0 = torch.empty_like(data)
+    mm.mm_loss_gradient(g, B, c, K, data, None, g0, l0, wr0)
+    mm.mm_forward(g, B, g0, K, wr0)
+    eta = 0.2 * float((g0.double() ** 2).sum() / (wr0.double() ** 2).sum())
+    del g0, wr0
+    kw = dict(eta=eta, momentum=0.5, mu_laplacian=1e-3 * scale, mu_l2=1e-4 * scale, max_iter=n_it, tol=1e-30, check_every=1)
+    mm.mm_iterate(g, B, K, data, None, c, v, torch.zeros(2, device="cuda", dtype=torch.float64), **{**kw, "max_iter": 2})   # warm-up (pool, clocks)
+    torch.cuda.synchronize()
+    c.zero_(); v.zero_()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = mm.mm_launch_count()
+    e0.record()
+    done = mm.mm_iterate(g, B, K, data, None, c, v, losses, **kw)
+    e1.record()
+    torch.cuda.synchronize()
+    launches = mm.mm_launch_count() - launches
+    it_ms = e0.elapsed_time(e1) / done
+    grad = torch.empty_like(c)
+    loss = torch.zeros(1, device="cuda", dtype=torch.float64)
+    wr = torch.empty_like(data)
+    for _ in range(3):
+        mm.mm_loss_gradient(g, B, c, K, data, None, grad, loss, wr)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n_it):
+        mm.mm_loss_gradient(g, B, c, K, data, None, grad, loss, wr)
+    e1.record()
+    torch.cuda.synchronize()
+    grad_ms = e0.elapsed_time(e1) / n_it
+    hist = losses.cpu().numpy()
+    line = {"what": "NEXT-3 device-resident regularised Nesterov iteration (PAPER.md:262-264, 270-272, 336-340)", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "regularisers": "Laplacian + L2", "momentum": 0.5, "eta": "0.2 x the exact line-search step of the first gradient", "stop_check_every": 1},
+            "iterations": int(done), "ms_per_iteration": it_ms, "bare_gradient_ms": grad_ms, "overhead_ms": it_ms - grad_ms,
+            "gpu_launches": int(launches), "host_syncs": "one 4-byte D2H per stop check",
+            "loss_first": float(hist[0]), "loss_last": float(hist[int(done) - 1])}
+    print(json.dumps(line))
+
+
 def sparse_extra(args):
     """`--sparse-extra`: NEXT-2 measurement (not the headline step).  Table V's largest basis (N = 162 directions, NN
     indicator functions) on a 100^3 volume, 240 projections (6 tilts x 40), 100^2 detector, D = 8:
@@ -486,6 +553,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true", help="also time mm_backproject (outside the step)")
+    ap.add_argument("--iterate-extra", action="store_true", help="time the NEXT-3 device-resident iteration (mm_iterate) against the bare gradient and exit")
     ap.add_argument("--sparse-extra", action="store_true", help="time the NEXT-2 sparse-plan calls against the dense ones (K = 162 NN basis) and exit")
     ap.add_argument("--record-traffic", metavar="NCU_RAW_CSV", help="store the kernels' DRAM bytes from an ncu raw-page csv and exit")
     ap.add_argument("--traffic-command", default="ncu --set full --clock-control none -k regex:john_forward|adjoint_brick ... python bench.py --steps 1 --warmup 3 --no-cpu-baseline; ncu -i <rep> --page raw --csv")
@@ -493,6 +561,9 @@ def main():
     cfg = synth.get_config(args.config)
     if args.record_traffic:
         record_traffic(args.record_traffic, cfg.name, args.traffic_command)
+        return
+    if args.iterate_extra:
+        iterate_extra(args)
         return
     if args.sparse_extra:
         sparse_extra(args)
