@@ -355,6 +355,26 @@ def ours(args, cfg):
         extras = {"mm_backproject_ms": e0.elapsed_time(e1) / args.steps,
                   "what": "basis^T + bilinear interpolation of the projection (PAPER.md:314), same wr as the step"}
 
+        def timed_extra(fn):
+            fn()
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(args.steps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / args.steps
+
+        # NEXT-4: the Huber-regressor step and the per-voxel derived quantities (Eq. 10-12)
+        delta = 3.0 * float(wr.abs().mean())
+        extras["mm_loss_gradient_huber_ms"] = timed_extra(lambda: mm.mm_loss_gradient_huber(g, B, vol, K, data, w, delta, grad, loss, wr))
+        n3 = tuple(cfg.shape)
+        dq = [torch.empty(n3 + t, device="cuda") for t in ((), (6,), (3,), (3, 3), ())]
+        extras["mm_derived_quantities_ms"] = timed_extra(lambda: mm.mm_derived_quantities(g, vol, K, *dq))
+        del dq
+        mm.mm_loss_gradient(g, B, vol, K, data, w, grad, loss, wr)          # leave grad / wr / loss as the step left them
+        torch.cuda.synchronize()
+
     # ---- end to end through the host-buffer C-ABI call (H2D of every input, D2H of gradient + loss, inside)
     e2e = None
     if rank == 0:
@@ -552,7 +572,7 @@ def main():
     ap.add_argument("--config", default="C5", choices=sorted(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--extras", action="store_true", help="also time mm_backproject (outside the step)")
+    ap.add_argument("--extras", action="store_true", help="also time mm_backproject, mm_loss_gradient_huber and mm_derived_quantities (outside the step)")
     ap.add_argument("--iterate-extra", action="store_true", help="time the NEXT-3 device-resident iteration (mm_iterate) against the bare gradient and exit")
     ap.add_argument("--sparse-extra", action="store_true", help="time the NEXT-2 sparse-plan calls against the dense ones (K = 162 NN basis) and exit")
     ap.add_argument("--record-traffic", metavar="NCU_RAW_CSV", help="store the kernels' DRAM bytes from an ncu raw-page csv and exit")
