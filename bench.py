@@ -50,7 +50,7 @@ def source_sha16():
     include: ties a stored ncu traffic figure to the code it was measured on"""
     import hashlib
     h = hashlib.sha256()
-    for name in ("mm_adjoint_brick.cu", "mm_internal.h", "mm_kernels.cu", "mm_ptx.cuh"):
+    for name in ("mm_adjoint_brick.cu", "mm_adjoint_brick_pair.cuh", "mm_internal.h", "mm_kernels.cu", "mm_ptx.cuh"):
         with open(os.path.join(ROOT, "paper_2504_16446_b200", "csrc", name), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
@@ -72,8 +72,8 @@ def record_traffic(csv_path, cfg_name, command):
         b = float(r[ir]) * unit[rows[1][ir]] + float(r[iw]) * unit[rows[1][iw]]
         if b != b:                                   # a launch ncu could not replay: no figure
             continue
-        for key in ("john_forward_kernel", "adjoint_brick_kernel"):
-            if key in r[ik]:
+        for key, match in (("john_forward_kernel", "john_forward_kernel"), ("adjoint_brick_kernel", "adjoint_brick")):
+            if match in r[ik]:                       # adjoint_brick_kernel or adjoint_brick_pair_kernel
                 ent[key + "_dram_bytes"] = int(b)
     out = os.path.join(ROOT, "profiles", "r02_traffic.json")
     tr = {}
