@@ -402,7 +402,7 @@ def ours(args, cfg):
                 "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "bound_note": "frac is the STREAMING MODEL (one volume pass per projection) against the HBM copy peak; "
                               "cross-projection L2 reuse keeps real DRAM traffic below the model (see dram_frac), and ncu "
-                              "(profiles/r02_ncu_c5_v5.md) shows no saturated unit on config 5 - L1 data pipe 83 %, DRAM 50 %, "
+                              "(profiles/r02_ncu_c5_v6.md) shows no saturated unit on config 5 - L1 data pipe 83 %, DRAM 50 %, "
                               "L2 37 %: the march is latency-bound at 16 warps per SM (DESIGN.md 5)",
                 "traffic": None, "dram_frac": None, "peak_source": peak_src, "ms_per_launch": fwd_ms,
                 "algorithmic_bytes_per_launch": fwd_bytes,
